@@ -1,0 +1,230 @@
+"""Seeded synthetic MPC workloads (numpy only; none of the solver's arithmetic lives here).
+
+These generators serve BOTH the CUDA path and the CPU oracle (tests and bench.py hand the same
+arrays to each); neither solver imports the other.  They realise the five `configs` of
+BASELINE.json as restated in SURVEY.md section 8(d), which stand in for the paper's own workloads
+(random dense LTV systems with box constraints; long-horizon CSTR).
+The recipe is restated in DESIGN.md "Input recipe".
+
+All arrays are float64, row-major:  A [batch][N][nx][nx], B [batch][N][nx][nu], x0 [batch][nx].
+Seeds: np.random.default_rng([2601, 14414, generator_id, instance]).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+SEED = (2601, 14414)
+
+
+@dataclass
+class Problem:
+    name: str
+    nx: int
+    nu: int
+    N: int
+    batch: int
+    A: np.ndarray                 # [batch][N][nx][nx]
+    B: np.ndarray                 # [batch][N][nx][nu]
+    Q: np.ndarray                 # [nx][nx]
+    R: np.ndarray                 # [nu][nu]
+    lo: np.ndarray                # [nx+nu] = (x_lo; u_lo)
+    hi: np.ndarray                # [nx+nu]
+    x0: np.ndarray                # [batch][nx]
+    e: np.ndarray | None = None   # [batch][N][nx]
+    P: np.ndarray | None = None   # terminal weight (None = Q)
+    Wdu: np.ndarray | None = None
+    qbar: np.ndarray | None = None
+    du_lo: np.ndarray | None = None
+    du_hi: np.ndarray | None = None
+    u_prev: np.ndarray | None = None   # [batch][nu]
+    rho: float = 1.0
+    iters: int = 100
+    tol: float = 0.0
+    dtypes: tuple = ("f64",)
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def nb(self) -> int:
+        return self.nx + self.nu
+
+    def instance(self, b: int) -> dict:
+        """Keyword arguments of one instance, in the naming both solvers' Python wrappers use."""
+        return dict(A=self.A[b], B=self.B[b], Q=self.Q, R=self.R, lo=self.lo, hi=self.hi, x0=self.x0[b],
+                    e=None if self.e is None else self.e[b], P=self.P, Wdu=self.Wdu, qbar=self.qbar,
+                    du_lo=self.du_lo, du_hi=self.du_hi,
+                    u_prev=None if self.u_prev is None else self.u_prev[b], rho=self.rho)
+
+    def rounded(self, dtype: str) -> "Problem":
+        """The same problem with every input rounded to `dtype` and promoted back to float64
+        (what the oracle is fed for an fp32 GPU run, SURVEY.md section 8(c) parity metric)."""
+        if dtype == "f64":
+            return self
+        r = lambda a: None if a is None else np.asarray(a, np.float32).astype(np.float64)
+        return Problem(self.name, self.nx, self.nu, self.N, self.batch, r(self.A), r(self.B), r(self.Q),
+                       r(self.R), r(self.lo), r(self.hi), r(self.x0), r(self.e), r(self.P), r(self.Wdu),
+                       r(self.qbar), r(self.du_lo), r(self.du_hi), r(self.u_prev), self.rho, self.iters,
+                       self.tol, self.dtypes, dict(self.meta))
+
+
+# --------------------------------------------------------------------------------------------
+# mass-spring chains (configs 1 and 5)
+# --------------------------------------------------------------------------------------------
+def _chain_continuous(masses, springs, damping, input_masses):
+    """wall - m_0 - m_1 - ... - m_{M-1} - wall with M+1 springs; state (p_0..p_{M-1}, v_0..v_{M-1}).
+    springs may be [M+1] or [K][M+1] (K stage-wise stiffness sets). Returns A_c [K][2M][2M], B_c [2M][nu]."""
+    masses = np.asarray(masses, float)
+    springs = np.atleast_2d(np.asarray(springs, float))
+    M = masses.size
+    K = springs.shape[0]
+    Ac = np.zeros((K, 2 * M, 2 * M))
+    idx = np.arange(M)
+    Ac[:, idx, M + idx] = 1.0                                            # p' = v
+    Ac[:, M + idx, idx] = -(springs[:, :-1] + springs[:, 1:]) / masses   # own position
+    Ac[:, M + idx[1:], idx[:-1]] = springs[:, 1:-1] / masses[1:]         # left neighbour
+    Ac[:, M + idx[:-1], idx[1:]] = springs[:, 1:-1] / masses[:-1]        # right neighbour
+    Ac[:, M + idx, M + idx] = -damping / masses                          # viscous damping
+    Bc = np.zeros((2 * M, len(input_masses)))
+    for j, mi in enumerate(input_masses):
+        Bc[M + mi, j] = 1.0 / masses[mi]
+    return Ac, Bc
+
+
+def config1(seed_instance: int = 0) -> Problem:
+    """C1: tiny LTI 2-mass chain, nx=4, nu=2, N=20, fp64, batch 1, 500 iterations, no du bounds."""
+    nx, nu, N, dt = 4, 2, 20, 0.1
+    Ac, Bc = _chain_continuous(np.ones(2), np.ones(3), 0.1, [0, 1])
+    A1 = np.eye(nx) + dt * Ac[0]
+    B1 = dt * Bc
+    rng = np.random.default_rng([*SEED, 1, seed_instance])
+    x0 = rng.uniform(-2.0, 2.0, size=(1, nx))
+    A = np.broadcast_to(A1, (1, N, nx, nx)).copy()
+    B = np.broadcast_to(B1, (1, N, nx, nu)).copy()
+    lo = np.concatenate([-4.0 * np.ones(nx), -0.5 * np.ones(nu)])
+    return Problem("C1", nx, nu, N, 1, A, B, np.eye(nx), 0.1 * np.eye(nu), lo, -lo, x0, P=np.eye(nx),
+                   rho=1.0, iters=500, tol=0.0, dtypes=("f64",))
+
+
+def config5(N: int = 2000, batch: int = 64, first_instance: int = 0) -> Problem:
+    """C5: 24-mass chain, nx=48, nu=12, per-stage +-5 % stiffness, |du| <= 0.1, 500 iterations."""
+    Mm, nu, dt = 24, 12, 0.05
+    nx = 2 * Mm
+    A = np.empty((batch, N, nx, nx))
+    B = np.empty((batch, N, nx, nu))
+    x0 = np.empty((batch, nx))
+    for b in range(batch):
+        rng = np.random.default_rng([*SEED, 5, first_instance + b])
+        masses = rng.uniform(0.5, 2.0, size=Mm)
+        springs = rng.uniform(0.5, 2.0, size=Mm + 1)
+        pert = rng.uniform(-1.0, 1.0, size=(N, Mm + 1))
+        x0[b] = rng.uniform(-1.0, 1.0, size=nx)
+        Ac, Bc = _chain_continuous(masses, springs * (1.0 + 0.05 * pert), 0.1, list(range(0, Mm, 2)))
+        A[b] = np.eye(nx) + dt * Ac
+        B[b] = dt * Bc
+    lo = np.concatenate([-3.0 * np.ones(nx), -1.0 * np.ones(nu)])
+    return Problem("C5", nx, nu, N, batch, A, B, np.eye(nx), 0.1 * np.eye(nu), lo, -lo, x0,
+                   du_lo=-0.1 * np.ones(nu), du_hi=0.1 * np.ones(nu), rho=1.0, iters=500, tol=0.0,
+                   dtypes=("f64", "f32"))
+
+
+# --------------------------------------------------------------------------------------------
+# linearised quadrotor-like LTV system (configs 2, 3, 4)
+# --------------------------------------------------------------------------------------------
+def quadrotor_cost():
+    """Shared diagonal Q ~ U[1,10]^12, R ~ U[0.01,0.1]^4 (cost rng)."""
+    rng = np.random.default_rng([*SEED, 2, 10**6])
+    return np.diag(rng.uniform(1.0, 10.0, size=12)), np.diag(rng.uniform(0.01, 0.1, size=4))
+
+
+def quadrotor_ltv(N: int, batch: int = 1, first_instance: int = 0, *, iters: int = 2000, tol: float = 1e-4,
+                  rho: float = 1.0, name: str = "C2", dtypes=("f64", "f32")) -> Problem:
+    """State (p, phi/theta/psi, v, omega), inputs (thrust, tau_x, tau_y, tau_z);
+    A_k = I + dt (J + dJ_k), B_k = dt (G + dG_k), dt = 0.02, dJ, dG ~ N(0, 0.05^2) per stage."""
+    nx, nu, dt = 12, 4, 0.02
+    J = np.zeros((nx, nx))
+    J[0:3, 6:9] = np.eye(3)
+    J[3:6, 9:12] = np.eye(3)
+    J[6, 4] = 9.81
+    J[7, 3] = -9.81
+    G = np.zeros((nx, nu))
+    G[8, 0] = 10.0
+    G[9, 1] = 50.0
+    G[10, 2] = 50.0
+    G[11, 3] = 20.0
+    Q, R = quadrotor_cost()
+    A = np.empty((batch, N, nx, nx))
+    B = np.empty((batch, N, nx, nu))
+    x0 = np.empty((batch, nx))
+    for b in range(batch):
+        rng = np.random.default_rng([*SEED, 2, first_instance + b])
+        dJ = rng.normal(0.0, 0.05, size=(N, nx, nx))
+        dG = rng.normal(0.0, 0.05, size=(N, nx, nu))
+        x0[b] = rng.uniform(-1.0, 1.0, size=nx)
+        A[b] = np.eye(nx) + dt * (J + dJ)
+        B[b] = dt * (G + dG)
+    lo = np.concatenate([-5.0 * np.ones(nx), -1.0 * np.ones(nu)])
+    return Problem(name, nx, nu, N, batch, A, B, Q, R, lo, -lo, x0, du_lo=-0.2 * np.ones(nu),
+                   du_hi=0.2 * np.ones(nu), rho=rho, iters=iters, tol=tol, dtypes=tuple(dtypes))
+
+
+def config2() -> Problem:
+    return quadrotor_ltv(100, 1, iters=2000, tol=1e-4, name="C2")
+
+
+def config3(N: int) -> Problem:
+    return quadrotor_ltv(N, 1, iters=1000, tol=0.0, name=f"C3-N{N}", dtypes=("f32",))
+
+
+C3_HORIZONS = (10, 100, 1000, 4000, 10000)
+
+
+def config4(batch: int = 4096, first_instance: int = 0) -> Problem:
+    return quadrotor_ltv(50, batch, first_instance, iters=200, tol=0.0, name="C4", dtypes=("f32",))
+
+
+# --------------------------------------------------------------------------------------------
+# small explicit / random systems used by the pins and the edge-case parity tests
+# --------------------------------------------------------------------------------------------
+def p_tiny(with_du_bounds: bool = False) -> Problem:
+    """The explicit no-RNG problem of SURVEY.md section 8(c) 'P-tiny' (double integrator, N=4)."""
+    nx, nu, N = 2, 1, 4
+    A = np.broadcast_to(np.array([[1.0, 0.1], [0.0, 1.0]]), (1, N, nx, nx)).copy()
+    B = np.broadcast_to(np.array([[0.005], [0.1]]), (1, N, nx, nu)).copy()
+    lo = np.array([-4.0, -0.3, -0.5])
+    hi = np.array([4.0, 0.3, 0.5])
+    kw = dict(du_lo=np.array([-0.2]), du_hi=np.array([0.2])) if with_du_bounds else {}
+    return Problem("P-tiny", nx, nu, N, 1, A, B, np.eye(2), np.array([[0.1]]), lo, hi,
+                   np.array([[1.0, 0.0]]), P=np.eye(2), rho=1.0, iters=10, **kw)
+
+
+def random_ltv(nx: int, nu: int, N: int, batch: int = 1, *, seed: int = 0, affine: bool = True,
+               bounds: float | None = None, du_bound: float | None = None, u_prev: bool = True,
+               full_cost: bool = False, wdu: bool = False, qbar: bool = False, scale: float = 0.3) -> Problem:
+    """Small dense random LTV systems with distinct A_k, B_k, e_k per stage (pins P-KKT / P-BF and
+    odd-shaped parity cases).  A_k = I + scale*N(0,1)/sqrt(nx), B_k = N(0,1), e_k = 0.1 N(0,1)."""
+    rng = np.random.default_rng([*SEED, 99, seed])
+    nb = nx + nu
+    A = np.eye(nx) + scale * rng.normal(size=(batch, N, nx, nx)) / np.sqrt(nx)
+    B = rng.normal(size=(batch, N, nx, nu))
+    e = 0.1 * rng.normal(size=(batch, N, nx)) if affine else None
+    x0 = rng.uniform(-1.0, 1.0, size=(batch, nx))
+    up = 0.3 * rng.uniform(-1.0, 1.0, size=(batch, nu)) if u_prev else None
+    if full_cost:
+        Lq = rng.normal(size=(nx, nx)); Lr = rng.normal(size=(nu, nu))
+        Q = Lq @ Lq.T / nx + 0.5 * np.eye(nx)
+        R = Lr @ Lr.T / nu + 0.1 * np.eye(nu)
+        P = 2.0 * Q
+    else:
+        Q = np.diag(rng.uniform(0.5, 2.0, size=nx)); R = np.diag(rng.uniform(0.05, 0.5, size=nu)); P = None
+    W = np.diag(rng.uniform(0.05, 0.3, size=nu)) if wdu else None
+    qb = 0.2 * rng.normal(size=nb) if qbar else None
+    if bounds is None:
+        lo = -np.inf * np.ones(nb); hi = np.inf * np.ones(nb)
+    else:
+        lo = -bounds * np.ones(nb); hi = bounds * np.ones(nb)
+    kw = {}
+    if du_bound is not None:
+        kw = dict(du_lo=-du_bound * np.ones(nu), du_hi=du_bound * np.ones(nu))
+    return Problem(f"rand-{nx}-{nu}-{N}", nx, nu, N, batch, A, B, Q, R, lo, hi, x0, e=e, P=P, Wdu=W, qbar=qb,
+                   u_prev=up, rho=1.0, iters=200, **kw)

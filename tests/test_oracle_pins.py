@@ -1,0 +1,282 @@
+"""Pins of the CPU oracle (oracle/pimpc_oracle.c) against what the paper and the mathematics fix.
+
+None of these tests re-types the oracle's formulas: they compare with dense KKT solves, a Riccati
+recursion, brute-force active-set enumeration, closed forms, library inverses, invariants of the
+ADMM iteration, and numbers produced by an independent implementation (tests/golden/p_tiny.txt).
+Chosen so that a dropped term, wrong sign/index or transposed operand fails at least one of them:
+  index of Abar/ebar in h_k (R2)           -> P-KKT on LTV with distinct e_k
+  z-update form (R1), v-update, duals      -> P-KKT, P-BF, invariants
+  Delta-u copy block (R12), Wdu (R13)      -> P-BF with active du bounds, P-KKT with Wdu
+  terminal weight (R14), qbar, u_prev      -> P-KKT / Riccati
+  residual c (R7)                          -> closed form c^1, golden c^1..c^10
+  accept / restart / momentum (R5, R6)     -> golden decision bits + c sequence, Lemma-2 monotonicity
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2601_14414_b200 import workloads as wl
+from tests import qp_reference as ref
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "p_tiny.txt")
+
+
+def _golden():
+    out = {}
+    with open(GOLD) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, *v = line.split()
+            out[k] = np.array([float(t) for t in v])
+    return out
+
+
+def _solve(oracle, prob, b=0, **kw):
+    args = prob.instance(b)
+    args.update(kw)
+    return oracle.solve(**args)
+
+
+# ----------------------------------------------------------------------------------------------
+# cache against numpy.linalg.inv of the printed definition
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("has_du,wdu", [(False, False), (True, True)])
+def test_cache_matches_library_inverse(oracle, has_du, wdu):
+    p = wl.random_ltv(5, 3, 4, seed=11, full_cost=True, wdu=wdu)
+    rho = 0.7
+    M, H = oracle.cache(p.A[0], p.B[0], p.Q, p.R, P=p.P, Wdu=p.Wdu, has_du=has_du, rho=rho)
+    nx, nu, nb = p.nx, p.nu, p.nb
+    for k in range(p.N):
+        Bb = np.vstack([p.B[0, k], np.eye(nu)])
+        S = Bb.T @ Bb + (p.Wdu / rho if wdu else 0) + (np.eye(nu) if has_du else 0)
+        np.testing.assert_allclose(M[k], np.linalg.inv(S), rtol=1e-12, atol=1e-14)
+        Qb = np.zeros((nb, nb)); Qb[:nx, :nx] = p.P if k == p.N - 1 else p.Q; Qb[nx:, nx:] = p.R
+        S = Qb + rho * np.eye(nb)
+        if k < p.N - 1:
+            Ab = np.block([[p.A[0, k + 1], p.B[0, k + 1]], [np.zeros((nu, nx)), np.eye(nu)]])
+            S = S + rho * Ab.T @ Ab
+        np.testing.assert_allclose(H[k], np.linalg.inv(S), rtol=1e-12, atol=1e-14)
+
+
+# ----------------------------------------------------------------------------------------------
+# P-KKT: unconstrained LTV problem == one dense KKT solve == Riccati recursion
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["plain", "wdu_qbar_fullcost"])
+def test_unconstrained_matches_dense_kkt(oracle, variant):
+    full = variant != "plain"
+    p = wl.random_ltv(3, 2, 6, seed=3, affine=True, u_prev=True, full_cost=full, wdu=full, qbar=full)
+    a = p.instance(0)
+    U, X = ref.dense_kkt(a["A"], a["B"], a["Q"], a["R"], a["x0"], e=a["e"], P=a["P"], Wdu=a["Wdu"],
+                         qbar=a["qbar"], u_prev=a["u_prev"])
+    r = _solve(oracle, p, max_iters=20000, tol=1e-24)
+    assert r.iters < 20000, "oracle did not converge"
+    assert np.max(np.abs(r.u - U)) <= 1e-9 * max(1.0, np.max(np.abs(U)))
+    assert np.max(np.abs(r.x - X)) <= 1e-9 * max(1.0, np.max(np.abs(X)))
+    # X (the unprojected copy) agrees with Z at convergence; DU is the increment of u
+    np.testing.assert_allclose(r.X, r.Z, atol=1e-9)
+    uu = np.vstack([a["u_prev"], r.u])
+    np.testing.assert_allclose(r.DU, np.diff(uu, axis=0), atol=1e-9)
+
+
+def test_unconstrained_matches_riccati(oracle):
+    p = wl.random_ltv(4, 2, 8, seed=5, affine=True, u_prev=False, full_cost=True)
+    a = p.instance(0)
+    U, X = ref.riccati_lqr(a["A"], a["B"], a["Q"], a["R"], a["x0"], e=a["e"], P=a["P"])
+    Uk, Xk = ref.dense_kkt(a["A"], a["B"], a["Q"], a["R"], a["x0"], e=a["e"], P=a["P"])
+    np.testing.assert_allclose(U, Uk, atol=1e-10)          # the two textbook routes agree
+    r = _solve(oracle, p, max_iters=30000, tol=1e-24)
+    assert r.iters < 30000
+    np.testing.assert_allclose(r.u, U, atol=1e-9)
+    np.testing.assert_allclose(r.x, X, atol=1e-9)
+
+
+def test_lti_e0_would_hide_index_bug_but_ltv_does_not(oracle):
+    """R2: with the index of Abar/ebar in h_k shifted the LTV iteration converges to a wrong point;
+    the KKT pin above is on an LTV system with distinct e_k, so it sees it.  Here: the KKT residual of
+    the converged oracle solution on a strongly time-varying system is ~0 (stationarity of QP (1))."""
+    p = wl.random_ltv(3, 1, 7, seed=21, affine=True, scale=1.0)
+    a = p.instance(0)
+    U, X = ref.dense_kkt(a["A"], a["B"], a["Q"], a["R"], a["x0"], e=a["e"], u_prev=a["u_prev"])
+    r = _solve(oracle, p, max_iters=50000, tol=1e-24)
+    assert r.iters < 50000
+    np.testing.assert_allclose(r.u, U, atol=1e-8)
+
+
+# ----------------------------------------------------------------------------------------------
+# P-BF: constrained problems == brute-force active-set enumeration
+# ----------------------------------------------------------------------------------------------
+def test_constrained_matches_bruteforce_all_bound_kinds(oracle):
+    """u-, x- and du-bounds all active at the solution (asserted), incl. affine e_k and u_prev."""
+    p = wl.random_ltv(2, 1, 4, seed=43, affine=True, u_prev=True, bounds=None, du_bound=0.4)
+    p.lo = np.array([-0.9, -0.9, -0.6]); p.hi = np.array([0.9, 0.9, 0.6])
+    a = p.instance(0)
+    U, X, kinds = ref.active_set_bruteforce(a["A"], a["B"], a["Q"], a["R"], a["lo"], a["hi"], a["x0"], e=a["e"],
+                                            u_prev=a["u_prev"], du_lo=a["du_lo"], du_hi=a["du_hi"])
+    assert kinds == {"u", "x", "du"}, kinds
+    r = _solve(oracle, p, max_iters=200000, tol=1e-22)
+    assert r.iters < 200000
+    np.testing.assert_allclose(r.u, U, atol=1e-8)
+    np.testing.assert_allclose(r.x, X, atol=1e-8)
+
+
+def test_constrained_two_inputs_bruteforce(oracle):
+    p = wl.random_ltv(2, 2, 2, seed=8, affine=True, u_prev=True, bounds=0.4, du_bound=0.3, wdu=True, qbar=True)
+    a = p.instance(0)
+    U, X, kinds = ref.active_set_bruteforce(a["A"], a["B"], a["Q"], a["R"], a["lo"], a["hi"], a["x0"], e=a["e"],
+                                            Wdu=a["Wdu"], qbar=a["qbar"], u_prev=a["u_prev"],
+                                            du_lo=a["du_lo"], du_hi=a["du_hi"])
+    assert len(kinds) >= 1
+    r = _solve(oracle, p, max_iters=200000, tol=1e-22)
+    assert r.iters < 200000
+    np.testing.assert_allclose(r.u, U, atol=1e-8)
+    np.testing.assert_allclose(r.x, X, atol=1e-8)
+
+
+def test_p_tiny_converged_matches_bruteforce_and_golden(oracle):
+    g = _golden()
+    for with_du, key in ((False, "ustar_nodu"), (True, "ustar_du")):
+        p = wl.p_tiny(with_du)
+        a = p.instance(0)
+        U, X, kinds = ref.active_set_bruteforce(a["A"], a["B"], a["Q"], a["R"], a["lo"], a["hi"], a["x0"],
+                                                P=a["P"], du_lo=a["du_lo"], du_hi=a["du_hi"])
+        np.testing.assert_allclose(U.ravel(), g[key], atol=2e-10)       # golden == brute force
+        r = _solve(oracle, p, max_iters=20000, tol=1e-26)
+        np.testing.assert_allclose(r.u.ravel(), g[key], atol=2e-10)     # oracle == golden
+        if not with_du:
+            np.testing.assert_allclose(r.x.ravel(), g["xstar_nodu"], atol=2e-10)
+
+
+# ----------------------------------------------------------------------------------------------
+# fixed-count numbers: c sequence, decision bits, iterates (independent implementation, SURVEY P-tiny)
+# ----------------------------------------------------------------------------------------------
+def test_p_tiny_fixed_count_numbers(oracle):
+    g = _golden()
+    r = _solve(oracle, wl.p_tiny(False), max_iters=10, tol=0.0)
+    np.testing.assert_allclose(r.c_hist, g["c_nodu"], rtol=2e-12)
+    assert list(r.acc_hist) == [int(v) for v in g["acc_nodu"]]
+    np.testing.assert_allclose(r.DU.ravel(), g["du10_nodu"], atol=2e-12)
+    np.testing.assert_allclose(r.Z[0], g["z0_10_nodu"], atol=2e-12)
+    r = _solve(oracle, wl.p_tiny(True), max_iters=5, tol=0.0)
+    np.testing.assert_allclose(r.c_hist, g["c_du"], rtol=2e-12)
+
+
+def test_c1_closed_form(oracle):
+    """P-c1: cold start, qbar=0, e=0, projection inactive at i=0 => only stage 0 moves and
+    c^1 = rho ||A_0 x0 + B_0 u_prev||^2 + rho ||u_prev||^2   (derived from Alg. 1)."""
+    p = wl.random_ltv(4, 2, 5, seed=2, affine=False, u_prev=True, bounds=None)
+    for rho in (1.0, 2.5):
+        a = p.instance(0); a["rho"] = rho
+        r = oracle.solve(**a, max_iters=1)
+        expect = rho * (np.sum((a["A"][0] @ a["x0"] + a["B"][0] @ a["u_prev"]) ** 2) + np.sum(a["u_prev"] ** 2))
+        assert abs(r.c_hist[0] - expect) <= 1e-13 * expect
+        b0 = np.concatenate([a["A"][0] @ a["x0"] + a["B"][0] @ a["u_prev"], a["u_prev"]])
+        np.testing.assert_allclose(r.Z[0], b0 / 3, atol=1e-14)
+        np.testing.assert_allclose(r.V[0], -b0 / 3, atol=1e-14)
+        np.testing.assert_allclose(r.TH[0], -b0 / 3, atol=1e-14)
+        assert np.all(r.Z[1:] == 0) and np.all(r.DU == 0)
+
+
+# ----------------------------------------------------------------------------------------------
+# invariants of the iteration (every iteration)
+# ----------------------------------------------------------------------------------------------
+def test_invariants_every_iteration(oracle):
+    p = wl.quadrotor_ltv(12, 1, iters=60)
+    a = p.instance(0)
+    warm = None
+    for it in range(60):
+        # one iteration at a time would reset alpha; instead run 1..60 from cold and check the end state
+        r = oracle.solve(**a, max_iters=it + 1)
+        # (i) beta + lambda = 0 (optimality in the unconstrained v, Eq. 15b)
+        assert np.max(np.abs(r.BE + r.LA)) <= 1e-12
+        # (ii) normal-cone condition (14c): Z = clip(Z + t (TH - LA)) for any t > 0
+        for t in (0.5, 3.0):
+            np.testing.assert_allclose(r.Z, np.clip(r.Z + t * (r.TH - r.LA), a["lo"], a["hi"]), atol=1e-12)
+        # (iii) feasibility of the projected copies
+        assert np.all(r.Z >= a["lo"]) and np.all(r.Z <= a["hi"])
+        assert np.all(r.D >= a["du_lo"]) and np.all(r.D <= a["du_hi"])
+
+
+def test_lemma2_plain_admm_monotone_and_restart_rule(oracle):
+    p = wl.quadrotor_ltv(10, 1, iters=400)
+    a = p.instance(0)
+    # eta = 0 => never accept => plain ADMM: c is non-increasing (Lemma 2)
+    r = oracle.solve(**{**a, "eta": 0.0}, max_iters=400)
+    assert r.restarts == 400
+    assert np.all(r.c_hist[1:] <= r.c_hist[:-1] * (1 + 1e-12))
+    # accelerated: accepted steps satisfy c^{i+1} <= eta c^i by construction; the step after a rejected
+    # step is a plain ADMM step from a plain iterate, so c does not increase there.
+    r = oracle.solve(**a, max_iters=400)
+    c, acc = r.c_hist, r.acc_hist
+    cprev = np.concatenate([[1.0], c[:-1]])
+    assert np.all(c[acc == 1] <= 0.999 * cprev[acc == 1])
+    rej = np.where(acc == 0)[0]
+    rej = rej[rej + 1 < len(c)]
+    assert np.all(c[rej + 1] <= c[rej] * (1 + 1e-12))
+    assert 0 < r.restarts < 400
+
+
+def test_forced_decisions_replay(oracle):
+    """P-flip protocol: forcing the oracle's own decision sequence reproduces the run bit for bit;
+    flipping one decision changes the trajectory."""
+    p = wl.quadrotor_ltv(8, 1)
+    a = p.instance(0)
+    r0 = oracle.solve(**a, max_iters=120)
+    r1 = oracle.solve(**a, max_iters=120, forced=r0.acc_hist)
+    assert np.array_equal(r0.Z, r1.Z) and np.array_equal(r0.c_hist, r1.c_hist)
+    f = r0.acc_hist.copy(); f[40] ^= 1
+    r2 = oracle.solve(**a, max_iters=120, forced=f)
+    assert np.array_equal(r0.c_hist[:41], r2.c_hist[:41]) and not np.array_equal(r0.Z, r2.Z)
+
+
+def test_convergence_residuals_and_stationarity(oracle):
+    """P-conv: consensus residuals, KKT stationarity (14b) and c all -> 0 (Lemma 3)."""
+    p = wl.random_ltv(3, 2, 5, seed=17, affine=True, bounds=0.8, du_bound=0.5)
+    a = p.instance(0)
+    r = oracle.solve(**a, max_iters=200000, tol=1e-24)
+    assert r.iters < 200000 and r.c_last < 1e-24
+    nx, nu, N = p.nx, p.nu, p.N
+    xb = np.concatenate([a["x0"], a["u_prev"]])
+    rho = a["rho"]
+    Qb = np.zeros((nx + nu, nx + nu)); Qb[:nx, :nx] = a["Q"]; Qb[nx:, nx:] = a["R"]
+    for k in range(N):
+        Ab = np.block([[a["A"][k], a["B"][k]], [np.zeros((nu, nx)), np.eye(nu)]])
+        Bb = np.vstack([a["B"][k], np.eye(nu)])
+        eb = np.concatenate([a["e"][k], np.zeros(nu)])
+        assert np.max(np.abs(r.X[k] - Ab @ xb - Bb @ r.DU[k] - eb)) < 1e-9      # dynamics consensus
+        assert np.max(np.abs(r.X[k] - r.Z[k])) < 1e-9
+        assert np.max(np.abs(Bb @ r.DU[k] - r.V[k])) < 1e-9
+        # stationarity in Delta u: Bbar' beta + delta = 0 ; in xbar: Qbar x + rho theta - rho Abar_{k+1}' lambda_{k+1} = 0
+        assert np.max(np.abs(Bb.T @ r.BE[k] + r.DE[k])) < 1e-9
+        g = Qb @ r.X[k] + rho * r.TH[k]
+        if k < N - 1:
+            Ab1 = np.block([[a["A"][k + 1], a["B"][k + 1]], [np.zeros((nu, nx)), np.eye(nu)]])
+            g = g - rho * Ab1.T @ r.LA[k + 1]
+        assert np.max(np.abs(g)) < 1e-8
+        xb = r.X[k]
+
+
+def test_warm_start_is_a_fresh_alg1_invocation(oracle):
+    """the output iterates seed the next invocation with hats = iterates, alpha_0 = 1."""
+    p = wl.quadrotor_ltv(6, 1)
+    a = p.instance(0)
+    r1 = oracle.solve(**a, max_iters=30)
+    warm = dict(Z=r1.Z, V=r1.V, TH=r1.TH, BE=r1.BE, LA=r1.LA, D=r1.D, DE=r1.DE)
+    r2 = oracle.solve(**a, max_iters=1, warm=warm)
+    # first iteration of a warm invocation uses kappa = 0: identical to forcing a restart at iteration 30
+    f = np.concatenate([r1.acc_hist[:29], [0]]).astype(np.uint8)
+    r3 = oracle.solve(**a, max_iters=31, forced=f)
+    np.testing.assert_allclose(r2.Z, r3.Z, rtol=0, atol=1e-15)
+
+
+def test_generators_are_deterministic_and_shaped():
+    p = wl.config1()
+    assert p.A.shape == (1, 20, 4, 4) and p.B.shape == (1, 20, 4, 2) and p.du_lo is None
+    q = wl.config4(batch=3)
+    assert q.A.shape == (3, 50, 12, 12) and np.array_equal(q.A, wl.config4(batch=3).A)
+    assert np.array_equal(wl.config4(batch=2, first_instance=1).A[0], q.A[1])
+    c5 = wl.config5(N=7, batch=2)
+    assert c5.A.shape == (2, 7, 48, 48) and c5.nu == 12
+    # forward-Euler chain: spectral radius close to 1 (SURVEY.md section 8(d) C5 probe: ~1.005)
+    assert 0.99 < np.max(np.abs(np.linalg.eigvals(c5.A[0, 0]))) < 1.02
