@@ -1,0 +1,166 @@
+/*
+ * pimpc.h -- C ABI of libpimpc.so: the accelerated, restarted ADMM iteration of piMPC
+ * (arxiv 2601.14414, Algorithm 1) over the velocity-form, construction-free
+ * MPC-QP (Problem (11)) as hand-written sm_100a CUDA.
+ *
+ * Conventions (all entry points)
+ *   - Plain C: opaque handle, plain pointers and sizes, no C++/torch types.
+ *   - Every data pointer may be HOST or DEVICE memory (resolved with cudaPointerGetAttributes).
+ *     Numeric arrays have the element type of the handle (`dtype`: double or float), row-major,
+ *     innermost index contiguous.  Scalars in structs are always double/int.
+ *   - Ownership: the library owns all device state.  Inputs are copied during the call: a host
+ *     buffer may be reused when the call returns; a device buffer once the handle's stream reaches
+ *     that point.  Outputs are caller-allocated.
+ *   - Errors: every function returns PIMPC_OK (0) or a negative code and never throws or aborts.
+ *     pimpc_last_error() gives a message.  A CUDA error poisons the handle (PIMPC_ESTATE later).
+ *   - A handle is not thread-safe; distinct handles are independent.  All work of a handle is
+ *     enqueued on its stream (opts.stream, a cudaStream_t; NULL = legacy default stream).
+ *   - There is no CPU fallback: without a CUDA device pimpc_create returns PIMPC_ECUDA.
+ *
+ * Notation (stage-indexed, k = 0..N-1, nb = nx+nu), as in the paper:
+ *   X[k] = xbar_{k+1}, Z[k] = z_{k+1}, V[k] = v_k, TH[k] = theta_k, BE[k] = beta_k,
+ *   LA[k] = lambda_k, DU[k] = Delta u_k; D[k], DE[k] = copy / scaled dual of the optional
+ *   Delta-u box (reading R12; active only when finite du bounds were supplied).
+ */
+#ifndef PIMPC_H
+#define PIMPC_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pimpc_s *pimpc_t;
+
+enum { PIMPC_OK = 0, PIMPC_EINVAL = -1, PIMPC_ENOMEM = -2, PIMPC_ECUDA = -3, PIMPC_ESTATE = -4,
+       PIMPC_ENOTPD = -5 };
+enum { PIMPC_F64 = 0, PIMPC_F32 = 1 };
+
+/* Iteration drivers.  AUTO picks by footprint. */
+enum {
+    PIMPC_ENGINE_AUTO = 0,
+    PIMPC_ENGINE_STAGED = 1,   /* one launch per step of Alg. 1 per iteration; any nx,nu; the A/B baseline */
+    PIMPC_ENGINE_RESIDENT = 2, /* one CTA per instance, all stage data on-chip for every iteration      */
+    PIMPC_ENGINE_STREAM = 3,   /* persistent CTAs stream per-stage blobs HBM->smem (bulk async copies)   */
+    PIMPC_ENGINE_COOP = 4      /* cooperative grid, data resident in smem, one grid barrier per iteration */
+};
+
+/* which = selector of pimpc_get_state / pimpc_set_state */
+enum { PIMPC_X = 0, PIMPC_Z = 1, PIMPC_V = 2, PIMPC_TH = 3, PIMPC_BE = 4, PIMPC_LA = 5, PIMPC_D = 6,
+       PIMPC_DE = 7, PIMPC_DU = 8 };
+
+typedef struct {
+    int dtype;        /* PIMPC_F64 | PIMPC_F32: arithmetic and I/O element type                      */
+    int engine;       /* PIMPC_ENGINE_*; AUTO = 0                                                     */
+    double rho;       /* ADMM penalty, > 0; 0 -> 1.0                                   */
+    double eta;       /* restart threshold; < 0 -> 0.999; 0 = plain ADMM           */
+    double c0;        /* c^0; 0 -> 1.0                                             */
+    int history;      /* > 0: keep (c^{i+1}, accept bit) of up to `history` iterations per instance   */
+    void *stream;     /* cudaStream_t on which all work of the handle is enqueued                     */
+} pimpc_opts;
+
+/* Per-instance result record written by pimpc_get (always double/int, host or device). */
+typedef struct {
+    double c;         /* c^{i+1} of the last executed iteration                    */
+    double alpha;     /* alpha after the last decision                             */
+    int iters;        /* iterations executed (i+1 at the break of step 5, else max_iters)             */
+    int restarts;     /* number of times step 7 (restart) was taken                                   */
+    int converged;    /* 1 if step 5 (c < tol) stopped the instance                                   */
+    int pad_;
+} pimpc_result;
+
+typedef struct {
+    int engine;               /* engine the last pimpc_solve used                                     */
+    int launches;             /* kernels launched by the last pimpc_solve (incl. the cache kernel)    */
+    long long total_launches; /* kernels launched by this handle since creation                       */
+    size_t device_bytes;      /* device memory owned by the handle                                    */
+    int sm_count;             /* SMs of the device                                                    */
+    int grid, block;          /* launch shape of the iteration kernel of the last solve               */
+    size_t smem_bytes;        /* dynamic shared memory of that kernel                                 */
+} pimpc_info;
+
+const char *pimpc_version(void);
+
+/* Fill `o` with defaults (f64, AUTO, rho=1, eta=0.999, c0=1, no history, default stream). */
+void pimpc_default_opts(pimpc_opts *o);
+
+/* Device bytes pimpc_create would allocate for these dimensions (0 on invalid arguments). */
+size_t pimpc_workspace_bytes(int nx, int nu, int N, int batch, const pimpc_opts *opts);
+
+/* Create a solver for `batch` independent MPC instances with nx states, nu inputs, horizon N
+ * (Problem (1)).  Cold start (all iterates 0, reading R9), e_k = 0, qbar = 0,
+ * u_prev = 0, no bounds (+-inf), Q = I, R = I until the setters are called.
+ * opts may be NULL (defaults).  EINVAL: nx,nu,N,batch <= 0, nx+nu > 128, rho <= 0, bad dtype. */
+int pimpc_create(pimpc_t *out, int nx, int nu, int N, int batch, const pimpc_opts *opts);
+int pimpc_destroy(pimpc_t h);
+
+/* Per-stage setter (BASELINE.json north_star).  b = instance, k = stage.
+ * A_k [nx][nx], B_k [nx][nu], e_k [nx] (dynamics (1b)); any may be NULL = unchanged.
+ * Q [nx][nx], R [nu][nu]: shared stage cost (Qbar = diag(Q,R)), NULL = unchanged.
+ * bounds [2][nx+nu] = (x_lo;u_lo) then (x_hi;u_hi) of the box Xbar = X x U, shared by
+ * all stages and instances unless per-instance bounds were set, NULL = unchanged.
+ * x0 [nx]: x(t) of instance b, NULL = unchanged. */
+int pimpc_set_stage(pimpc_t h, int b, int k, const void *A_k, const void *B_k, const void *e_k,
+                    const void *Q, const void *R, const void *bounds, const void *x0);
+
+/* Bulk setter: A [batch][N][nx][nx], B [batch][N][nx][nu], e [batch][N][nx] or NULL (= keep). */
+int pimpc_set_stages(pimpc_t h, const void *A, const void *B, const void *e);
+
+/* Cost.  Q [nx][nx] = C'W_y C and R [nu][nu] = W_u symmetric PSD.
+ * P [nx][nx] or NULL: terminal weight used instead of Q at stage N-1 (R14; NULL = Q).
+ * Wdu [nu][nu] or NULL: weight on Delta u (R13; NULL = 0).
+ * qbar [nx+nu] or NULL: linear term col(C'W_y r_y, W_u r_u) (NULL = 0).
+ * per_instance != 0: each array has a leading [batch] dimension. */
+int pimpc_set_cost(pimpc_t h, const void *Q, const void *R, const void *P, const void *Wdu,
+                   const void *qbar, int per_instance);
+
+/* Box constraints.  lo, hi [nx+nu] = (x_lo;u_lo), (x_hi;u_hi); +-inf = unbounded.
+ * du_lo, du_hi [nu] or both NULL: box on Delta u (R12).  Passing finite du bounds enables the
+ * D/DE consensus block; passing NULL disables it (the iteration is then exactly Alg. 1).
+ * per_instance != 0: leading [batch] dimension.  EINVAL if any lo > hi or a NaN. */
+int pimpc_set_bounds(pimpc_t h, const void *lo, const void *hi, const void *du_lo, const void *du_hi,
+                     int per_instance);
+
+/* x0 [batch][nx] = x(t); u_prev [batch][nu] = u(t-1) or NULL (= 0)  (xbar_0, R10). */
+int pimpc_set_x0(pimpc_t h, const void *x0, const void *u_prev);
+
+/* One invocation of Algorithm 1 per instance from the current iterates (hats = iterates,
+ * alpha_0 = 1, c^0 = c0): recomputes the cache {M_k, H_k} if stage
+ * data, cost or rho changed, then runs up to max_iters iterations; an instance stops early when
+ * c^{i+1} < tol (step 5); tol <= 0 runs exactly max_iters.  Asynchronous on the
+ * handle's stream; errors detected on the device (non-finite input, matrix not positive definite)
+ * are reported by the next pimpc_get / pimpc_sync.  max_iters == 0 only refreshes the cache. */
+int pimpc_solve(pimpc_t h, int max_iters, double tol);
+
+/* Results of the last solve (synchronises the stream).  Any pointer may be NULL.
+ * x [batch][N][nx] = x_1..x_N and u [batch][N][nu] = u_0..u_{N-1} are read from Z (bound-feasible);
+ * du [batch][N][nu] = Delta u_0..; res [batch] pimpc_result. */
+int pimpc_get(pimpc_t h, void *x, void *u, void *du, pimpc_result *res);
+
+/* Raw iterates, [batch][N][nx+nu] (X,Z,V,TH,BE,LA) or [batch][N][nu] (D,DE,DU), for parity checks and
+ * warm starts.  get synchronises.  set replaces one array of the current iterate
+ * (X and DU are outputs only: EINVAL). */
+int pimpc_get_state(pimpc_t h, int which, void *out);
+int pimpc_set_state(pimpc_t h, int which, const void *in);
+
+/* History of the last solve: c [batch][cap] (double), accepted [batch][cap] (unsigned char),
+ * cap = opts.history; entries beyond an instance's `iters` are 0.  Synchronises. */
+int pimpc_get_history(pimpc_t h, double *c, unsigned char *accepted);
+
+/* The cache of the last solve, for parity checks: M [batch][N][nu][nu], H [batch][N][nb][nb]. */
+int pimpc_get_cache(pimpc_t h, void *M, void *H);
+
+/* Cold start: all iterates = 0 (R9). */
+int pimpc_reset(pimpc_t h);
+
+/* Wait for the handle's stream; returns a deferred device-side error if one was raised. */
+int pimpc_sync(pimpc_t h);
+
+int pimpc_get_info(pimpc_t h, pimpc_info *info);
+const char *pimpc_last_error(pimpc_t h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIMPC_H */

@@ -1,0 +1,274 @@
+// a0: the per-solve cache of Algorithm 1 (Remark 5), plus the small
+// bookkeeping kernels (begin / gather / state I/O).  One CTA per (instance, stage); the SPD
+// matrix lives in shared memory in double precision whatever the handle's dtype and is inverted
+// in place by Gauss-Jordan exchange steps without pivoting (safe for SPD matrices).
+#include "pimpc_internal.h"
+
+namespace {
+
+// In-place inverse of the SPD n x n matrix S (shared memory, row-major).  All threads call.
+// Returns false (uniformly) if a pivot is not positive / finite.
+__device__ bool gj_invert(double *S, double *colb, double *rowb, int n)
+{
+    const int tid = threadIdx.x, nt = blockDim.x;
+    bool ok = true;
+    for (int p = 0; p < n; ++p) {
+        __syncthreads();
+        const double piv = S[p * n + p];
+        if (!(piv > 0.0) || !isfinite(piv)) ok = false;
+        for (int t = tid; t < n; t += nt) { colb[t] = S[t * n + p]; rowb[t] = S[p * n + t]; }
+        __syncthreads();
+        const double inv = 1.0 / piv;
+        for (int idx = tid; idx < n * n; idx += nt) {
+            const int i = idx / n, j = idx - i * n;
+            double v;
+            if (i == p) v = (j == p) ? inv : rowb[j] * inv;
+            else if (j == p) v = -colb[i] * inv;
+            else v = S[idx] - colb[i] * rowb[j] * inv;
+            S[idx] = v;
+        }
+    }
+    __syncthreads();
+    return ok;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_setup(Prob<T> p)
+{
+    extern __shared__ double sm[];
+    const int nx = p.nx, nu = p.nu, nb = p.nb, N = p.N;
+    double *S = sm, *colb = S + nb * nb, *rowb = colb + nb;
+    const int k = blockIdx.x, b = blockIdx.y;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const bool last = (k == N - 1);
+    const T *A1 = p.A + ((size_t)b * N + (last ? k : k + 1)) * nx * nx;
+    const T *B1 = p.B + ((size_t)b * N + (last ? k : k + 1)) * nx * nu;
+    const T *Qx = (last && p.P) ? p.P + (size_t)b * p.cost_stride_q : p.Q + (size_t)b * p.cost_stride_q;
+    const T *Rx = p.R + (size_t)b * p.cost_stride_r;
+    const double rho = p.rho;
+    bool finite = true;
+
+    // H_k = (Qbar + rho I + rho Abar_{k+1}^T Abar_{k+1})^-1, k < N-1;  (Qbar_N + rho I)^-1, k = N-1
+    for (int idx = tid; idx < nb * nb; idx += nt) {
+        const int i = idx / nb, j = idx - i * nb;
+        double s = 0.0;
+        if (i < nx && j < nx) s = (double)Qx[i * nx + j];
+        else if (i >= nx && j >= nx) s = (double)Rx[(i - nx) * nu + (j - nx)];
+        if (i == j) s += rho;
+        if (!last) {
+            double a = (i == j && i >= nx) ? 1.0 : 0.0;          // the [0 I] rows of Abar
+            for (int r = 0; r < nx; ++r) {
+                const double ai = (i < nx) ? (double)A1[r * nx + i] : (double)B1[r * nu + (i - nx)];
+                const double aj = (j < nx) ? (double)A1[r * nx + j] : (double)B1[r * nu + (j - nx)];
+                a += ai * aj;
+            }
+            s += rho * a;
+        }
+        if (!isfinite(s)) finite = false;
+        S[idx] = s;
+    }
+    bool ok = gj_invert(S, colb, rowb, nb);
+    T *Hk = p.H + ((size_t)b * N + k) * nb * nb;
+    for (int idx = tid; idx < nb * nb; idx += nt) {
+        const int i = idx / nb, j = idx - i * nb;
+        Hk[idx] = (T)(0.5 * (S[idx] + S[j * nb + i]));            // exactly symmetric
+    }
+    __syncthreads();
+
+    // M_k = (B_k^T B_k + I [+ Wdu/rho] [+ I])^-1  so that J_k = M_k Bbar_k^T  (R12, R13)
+    const T *Bk = p.B + ((size_t)b * N + k) * nx * nu;
+    const T *Ak = p.A + ((size_t)b * N + k) * nx * nx;
+    for (int idx = tid; idx < nx * nx; idx += nt)
+        if (!isfinite((double)Ak[idx])) finite = false;
+    for (int idx = tid; idx < nu * nu; idx += nt) {
+        const int i = idx / nu, j = idx - i * nu;
+        double s = (i == j) ? 1.0 : 0.0;
+        for (int r = 0; r < nx; ++r) s += (double)Bk[r * nu + i] * (double)Bk[r * nu + j];
+        if (p.Wdu) s += (double)p.Wdu[(size_t)b * p.cost_stride_r + idx] / rho;
+        if (p.has_du && i == j) s += 1.0;
+        if (!isfinite(s)) finite = false;
+        S[idx] = s;
+    }
+    ok = gj_invert(S, colb, rowb, nu) && ok;
+    T *Mk = p.M + ((size_t)b * N + k) * nu * nu;
+    for (int idx = tid; idx < nu * nu; idx += nt) {
+        const int i = idx / nu, j = idx - i * nu;
+        Mk[idx] = (T)(0.5 * (S[idx] + S[j * nu + i]));
+    }
+    if (!finite) atomicOr(p.err, PIMPC_DEVERR_NONFINITE);
+    else if (!ok && tid == 0) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
+}
+
+// Input of Alg. 1: hats = iterates (i_prev = i_cur), alpha_0 = 1, c^0 = c0.
+template <typename T>
+__global__ void k_begin(Prob<T> p)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= p.batch) return;
+    InstCtl c = p.ctl[b];
+    c.alpha = 1.0; c.c_prev = p.c0; c.c_last = p.c0; c.kappa = 0.0;
+    c.i_prev = c.i_cur; c.i_new = (c.i_cur + 1) % 3;
+    c.done = 0; c.iters = 0; c.restarts = 0;
+    p.ctl[b] = c;
+    bool finite = true;
+    for (int i = 0; i < p.nx; ++i) if (!isfinite((double)p.x0[(size_t)b * p.nx + i])) finite = false;
+    for (int i = 0; i < p.nu; ++i) if (!isfinite((double)p.uprev[(size_t)b * p.nu + i])) finite = false;
+    if (!finite) atomicOr(p.err, PIMPC_DEVERR_NONFINITE);
+    if (p.hist_c)
+        for (int i = 0; i < p.hist_cap; ++i) { p.hist_c[(size_t)b * p.hist_cap + i] = 0.0; p.hist_a[(size_t)b * p.hist_cap + i] = 0; }
+}
+
+template <typename T>
+__global__ void k_gather(Prob<T> p, T *x, T *u, T *du, pimpc_result *res)
+{
+    const int b = blockIdx.y;
+    const InstCtl c = p.ctl[b];
+    const T *S = p.S + (size_t)c.i_cur * p.buf_stride;
+    const int per = p.nb + p.nu;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < p.N * per; idx += gridDim.x * blockDim.x) {
+        const int k = idx / per, i = idx - k * per;
+        if (i < p.nb) {
+            const T z = S[p.st(b, k) + i];
+            if (i < p.nx) { if (x) x[((size_t)b * p.N + k) * p.nx + i] = z; }
+            else if (u) u[((size_t)b * p.N + k) * p.nu + (i - p.nx)] = z;
+        } else if (du) {
+            du[((size_t)b * p.N + k) * p.nu + (i - p.nb)] = p.DU[((size_t)b * p.N + k) * p.nu + (i - p.nb)];
+        }
+    }
+    if (res && blockIdx.x == 0 && threadIdx.x == 0) {
+        pimpc_result r;
+        r.c = c.c_last; r.alpha = c.alpha; r.iters = c.iters; r.restarts = c.restarts;
+        r.converged = c.done; r.pad_ = 0;
+        res[b] = r;
+    }
+}
+
+// which: PIMPC_X.. ; set = 0: state -> dense buffer, 1: dense buffer -> state (current iterate).
+template <typename T>
+__global__ void k_state_io(Prob<T> p, int which, T *buf, int set)
+{
+    const int b = blockIdx.y;
+    const InstCtl c = p.ctl[b];
+    T *S = p.S + (size_t)c.i_cur * p.buf_stride;
+    int w, off = 0;
+    T *dense = nullptr;
+    switch (which) {
+    case PIMPC_X: w = p.nb; dense = p.X; break;
+    case PIMPC_DU: w = p.nu; dense = p.DU; break;
+    case PIMPC_Z: w = p.nb; off = p.oZ(); break;
+    case PIMPC_V: w = p.nb; off = p.oV(); break;
+    case PIMPC_TH: w = p.nb; off = p.oTH(); break;
+    case PIMPC_BE: w = p.nb; off = p.oBE(); break;
+    case PIMPC_LA: w = p.nb; off = p.oLA(); break;
+    case PIMPC_D: w = p.nu; off = p.oD(); break;
+    default: w = p.nu; off = p.oDE(); break;
+    }
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < p.N * w; idx += gridDim.x * blockDim.x) {
+        const int k = idx / w, i = idx - k * w;
+        T *src = dense ? dense + ((size_t)b * p.N + k) * w + i : S + p.st(b, k) + off + i;
+        T *ext = buf + ((size_t)b * p.N + k) * w + i;
+        if (set) *src = *ext; else *ext = *src;
+    }
+}
+
+__global__ void k_zero_ctl(InstCtl *ctl, int batch, double c0)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    InstCtl c;
+    c.alpha = 1.0; c.c_prev = c0; c.c_last = c0; c.kappa = 0.0;
+    c.i_prev = 0; c.i_cur = 0; c.i_new = 1; c.done = 0; c.iters = 0; c.restarts = 0; c.pad_[0] = c.pad_[1] = 0;
+    ctl[b] = c;
+}
+
+} // namespace
+
+template <typename T>
+Prob<T> make_prob(pimpc_s *h, double tol)
+{
+    Prob<T> p{};
+    p.nx = h->nx; p.nu = h->nu; p.nb = h->nb; p.N = h->N; p.batch = h->batch; p.rec = h->rec;
+    p.has_du = h->has_du; p.has_e = h->has_e;
+    p.A = (const T *)h->A; p.B = (const T *)h->B; p.e = h->has_e ? (const T *)h->e : nullptr;
+    p.x0 = (const T *)h->x0; p.uprev = (const T *)h->uprev;
+    p.Q = (const T *)h->Q; p.R = (const T *)h->R;
+    p.P = h->has_P ? (const T *)h->P : nullptr;
+    p.Wdu = h->has_wdu ? (const T *)h->Wdu : nullptr;
+    p.qbar = (const T *)h->qbar;
+    p.cost_stride_q = h->cost_per_instance ? h->nx * h->nx : 0;
+    p.cost_stride_r = h->cost_per_instance ? h->nu * h->nu : 0;
+    p.qbar_stride = h->cost_per_instance ? h->nb : 0;
+    p.lo = (const T *)h->lo; p.hi = (const T *)h->hi; p.dlo = (const T *)h->dlo; p.dhi = (const T *)h->dhi;
+    p.bnd_stride = h->bnd_per_instance ? h->nb : 0;
+    p.dbnd_stride = h->bnd_per_instance ? h->nu : 0;
+    p.H = (T *)h->H; p.M = (T *)h->M; p.S = (T *)h->S;
+    p.buf_stride = (size_t)h->batch * h->N * h->rec;
+    p.X = (T *)h->X; p.DU = (T *)h->DU;
+    p.ctl = h->ctl; p.partial = h->partial; p.nparts = 0;
+    p.hist_c = h->hist_c; p.hist_a = h->hist_a; p.hist_cap = h->hist_cap;
+    p.err = h->err;
+    p.rho = h->rho; p.eta = h->eta; p.tol = tol; p.c0 = h->c0;
+    return p;
+}
+template Prob<float> make_prob<float>(pimpc_s *, double);
+template Prob<double> make_prob<double>(pimpc_s *, double);
+
+template <typename T>
+static int setup_t(pimpc_s *h)
+{
+    Prob<T> p = make_prob<T>(h, 0.0);
+    const size_t smem = ((size_t)h->nb * h->nb + 2 * h->nb) * sizeof(double);
+    if (smem > 48 * 1024)
+        PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(k_setup<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int threads = h->nb * h->nb >= 1024 ? 256 : 128;
+    k_setup<T><<<dim3(h->N, h->batch), threads, smem, h->stream>>>(p);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 1;
+}
+
+int launch_setup(pimpc_s *h) { return h->dtype == PIMPC_F64 ? setup_t<double>(h) : setup_t<float>(h); }
+
+int launch_begin(pimpc_s *h)
+{
+    const int th = 128, bl = (h->batch + th - 1) / th;
+    if (h->dtype == PIMPC_F64) k_begin<double><<<bl, th, 0, h->stream>>>(make_prob<double>(h, 0.0));
+    else k_begin<float><<<bl, th, 0, h->stream>>>(make_prob<float>(h, 0.0));
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 1;
+}
+
+int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res)
+{
+    const int work = h->N * (h->nb + h->nu);
+    const int th = 256, bl = min(64, (work + th - 1) / th);
+    if (h->dtype == PIMPC_F64)
+        k_gather<double><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<double>(h, 0.0), (double *)x, (double *)u, (double *)du, res);
+    else
+        k_gather<float><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<float>(h, 0.0), (float *)x, (float *)u, (float *)du, res);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 1;
+}
+
+int launch_state_io(pimpc_s *h, int which, void *buf, int set)
+{
+    const int work = h->N * h->nb;
+    const int th = 256, bl = min(64, (work + th - 1) / th);
+    if (h->dtype == PIMPC_F64)
+        k_state_io<double><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<double>(h, 0.0), which, (double *)buf, set);
+    else
+        k_state_io<float><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<float>(h, 0.0), which, (float *)buf, set);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 1;
+}
+
+int launch_zero_state(pimpc_s *h)
+{
+    const size_t sbytes = 3 * (size_t)h->batch * h->N * h->rec * h->esz;
+    PIMPC_CUDA_TRY(h, cudaMemsetAsync(h->S, 0, sbytes, h->stream));
+    PIMPC_CUDA_TRY(h, cudaMemsetAsync(h->X, 0, (size_t)h->batch * h->N * h->nb * h->esz, h->stream));
+    PIMPC_CUDA_TRY(h, cudaMemsetAsync(h->DU, 0, (size_t)h->batch * h->N * h->nu * h->esz, h->stream));
+    const int th = 128, bl = (h->batch + th - 1) / th;
+    k_zero_ctl<<<bl, th, 0, h->stream>>>(h->ctl, h->batch, h->c0);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 1;
+}

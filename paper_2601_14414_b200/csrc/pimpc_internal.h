@@ -1,0 +1,119 @@
+// Internal declarations of libpimpc.so (not part of the ABI; see include/pimpc.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "../../include/pimpc.h"
+
+// Per-instance control block of Algorithm 1 (device memory, one per instance).
+// alpha, c_prev: state of the accept/restart test; kappa = (alpha_i-1)/alpha_{i+1}
+// is the momentum used to form the hats of the NEXT iteration from (cur, prev).
+// i_prev/i_cur/i_new: which of the three rotating state buffers hold the previous iterate, the
+// current iterate and the one being written.  After a solve i_cur holds the returned iterate.
+struct InstCtl {
+    double alpha, c_prev, c_last, kappa;
+    int i_prev, i_cur, i_new;
+    int done, iters, restarts;
+    int pad_[2];
+};
+static_assert(sizeof(InstCtl) == 64, "InstCtl must be 64 bytes");
+
+// Device error flag bits (raised by kernels, reported by pimpc_sync / pimpc_get).
+enum { PIMPC_DEVERR_NONFINITE = 1, PIMPC_DEVERR_NOTPD = 2 };
+
+// Geometry and pointers handed to every kernel by value.  T = float or double.
+// State record of one (instance, stage): [Z(nb) V(nb) TH(nb) BE(nb) LA(nb) D(nu) DE(nu) pad] = rec elements.
+template <typename T>
+struct Prob {
+    int nx, nu, nb, N, batch, rec;
+    int has_du, has_e;
+    const T *A, *B, *e;              // [batch][N][nx][nx], [batch][N][nx][nu], [batch][N][nx] or null
+    const T *x0, *uprev;             // [batch][nx], [batch][nu]
+    const T *Q, *R, *P, *Wdu, *qbar; // cost; P, Wdu may be null; stride 0 = shared by all instances
+    int cost_stride_q, cost_stride_r, qbar_stride;
+    const T *lo, *hi, *dlo, *dhi;    // bounds; strides 0 = shared
+    int bnd_stride, dbnd_stride;
+    T *H, *M;                        // cache: [batch][N][nb][nb] (symmetric), [batch][N][nu][nu]
+    T *S;                            // 3 rotating buffers of [batch][N][rec]
+    size_t buf_stride;               // elements between buffers
+    T *X, *DU;                       // [batch][N][nb], [batch][N][nu]
+    InstCtl *ctl;                    // [batch]
+    double *partial;                 // [batch][nparts] partial sums of c (before the factor rho)
+    int nparts;
+    double *hist_c;                  // [batch][hist_cap] or null
+    unsigned char *hist_a;
+    int hist_cap;
+    int *err;                        // device error flag
+    double rho, eta, tol, c0;
+
+    __host__ __device__ size_t st(int b, int k) const { return ((size_t)b * N + k) * rec; }
+    __host__ __device__ int oZ() const { return 0; }
+    __host__ __device__ int oV() const { return nb; }
+    __host__ __device__ int oTH() const { return 2 * nb; }
+    __host__ __device__ int oBE() const { return 3 * nb; }
+    __host__ __device__ int oLA() const { return 4 * nb; }
+    __host__ __device__ int oD() const { return 5 * nb; }
+    __host__ __device__ int oDE() const { return 5 * nb + nu; }
+};
+
+struct pimpc_s {
+    int nx = 0, nu = 0, nb = 0, N = 0, batch = 0, rec = 0;
+    int dtype = PIMPC_F64;
+    size_t esz = 8;
+    int engine_req = PIMPC_ENGINE_AUTO;
+    double rho = 1.0, eta = 0.999, c0 = 1.0;
+    int hist_cap = 0;
+    cudaStream_t stream = nullptr;
+    int device = 0, sm_count = 0;
+    size_t smem_optin = 0;
+
+    // device buffers (element type = dtype unless noted)
+    void *A = nullptr, *B = nullptr, *e = nullptr, *x0 = nullptr, *uprev = nullptr;
+    void *Q = nullptr, *R = nullptr, *P = nullptr, *Wdu = nullptr, *qbar = nullptr;
+    int cost_per_instance = 0;
+    void *lo = nullptr, *hi = nullptr, *dlo = nullptr, *dhi = nullptr;
+    int bnd_per_instance = 0;
+    int has_du = 0, has_e = 0, has_P = 0, has_wdu = 0;
+    void *H = nullptr, *M = nullptr, *S = nullptr, *X = nullptr, *DU = nullptr;
+    InstCtl *ctl = nullptr;
+    double *partial = nullptr;
+    int nparts_cap = 0;
+    double *hist_c = nullptr;
+    unsigned char *hist_a = nullptr;
+    int *err = nullptr;
+    // scratch of the STAGED engine (allocated on first use)
+    void *hat = nullptr, *W = nullptr, *G = nullptr, *rhs = nullptr;
+    // engine-private storage (packed blobs of the STREAM engine etc.)
+    void *blob = nullptr;
+    size_t blob_stride = 0;
+    bool blob_dirty = true;
+
+    bool cache_dirty = true;
+    size_t device_bytes = 0;
+    pimpc_info info{};
+    std::string errmsg;
+    int poisoned = 0;
+};
+
+// ---- kernels / engine entry points (each returns the number of kernels it launched, <0 on error) ----
+template <typename T> Prob<T> make_prob(pimpc_s *h, double tol);
+
+int launch_setup(pimpc_s *h);                       // a0: cache {M_k, H_k}
+int launch_begin(pimpc_s *h);                       // Alg. 1 input: alpha=1, c_prev=c0, hats=iterates
+int run_staged(pimpc_s *h, int iters, double tol);  // v0 engine
+int run_resident(pimpc_s *h, int iters, double tol);
+bool resident_supported(const pimpc_s *h, std::string *why);
+int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res_dev);
+int launch_state_io(pimpc_s *h, int which, void *buf_dev, int set);
+int launch_zero_state(pimpc_s *h);
+
+#define PIMPC_CUDA_TRY(h, expr)                                                         \
+    do {                                                                                \
+        cudaError_t err__ = (expr);                                                     \
+        if (err__ != cudaSuccess) {                                                     \
+            (h)->errmsg = std::string(#expr) + ": " + cudaGetErrorString(err__);        \
+            (h)->poisoned = 1;                                                          \
+            return PIMPC_ECUDA;                                                         \
+        }                                                                               \
+    } while (0)

@@ -1,0 +1,139 @@
+"""Parity harness: libpimpc (CUDA, through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Protocol (SURVEY.md section 8(c) P-flip):
+  * both sides log (c^{i+1}, accept bit) per iteration and instance;
+  * identical decision sequences -> compare every iterate array element by element;
+  * if they first differ at i*, the oracle's margin |c/(eta c_prev) - 1| at i* must be below
+    tau (1e-11 fp64, 1e-5 fp32), i.e. a genuine floating-point near-tie -- otherwise FAIL --
+    and the oracle is re-run with the GPU's decision sequence forced (never the other way round);
+  * fp32 runs: the oracle is fed the fp32-rounded inputs promoted to double.
+Metric: per array and instance  max|g - o| / max(max|o|, tiny)  <= 1e-9 (fp64) / 1e-4 (fp32);
+c relative <= 1e-7 / 1e-3 (BASELINE.json north_star).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+TOL = {"f64": 1e-9, "f32": 1e-4}
+TOL_C = {"f64": 1e-7, "f32": 1e-3}
+TAU = {"f64": 1e-11, "f32": 1e-5}
+ARRAYS = ("Z", "V", "TH", "BE", "LA", "X", "DU")
+
+
+def relerr(g, o):
+    g = np.asarray(g, np.float64); o = np.asarray(o, np.float64)
+    return float(np.max(np.abs(g - o)) / max(float(np.max(np.abs(o))), 1e-300)) if o.size else 0.0
+
+
+def gpu_run(pimpc, prob, dtype, *, engine="auto", iters=None, tol=None, history=True, instances=None,
+            warm=None, eta=0.999):
+    """Run libpimpc on `prob` (all instances).  Returns dict of numpy results."""
+    iters = prob.iters if iters is None else iters
+    tol = prob.tol if tol is None else tol
+    s = pimpc.Solver(prob.nx, prob.nu, prob.N, prob.batch, dtype=dtype, engine=engine, rho=prob.rho, eta=eta,
+                     history=iters if history else 0)
+    s.set_problem(prob)
+    if warm is not None:
+        for k, v in warm.items():
+            s.set_state(k, v)
+    s.solve(iters, tol)
+    out = {}
+    x, u, du, res = s.get()
+    out.update(x=x, u=u, du=du, res=res)
+    names = ARRAYS + (("D", "DE") if prob.du_lo is not None else ())
+    for n in names:
+        out[n] = s.get_state(n)
+    if history:
+        out["c_hist"], out["acc_hist"] = s.get_history()
+    out["info"] = s.get_info()
+    s.close()
+    return out
+
+
+def oracle_run(oracle, prob, dtype, b, *, iters=None, tol=None, forced=None, warm=None, eta=0.999):
+    p = prob.rounded(dtype)
+    kw = p.instance(b)
+    if warm is not None:
+        kw["warm"] = {k: np.asarray(v[b], np.float64) for k, v in warm.items()}
+    return oracle.solve(**kw, eta=eta, max_iters=prob.iters if iters is None else iters,
+                        tol=prob.tol if tol is None else tol, forced=forced)
+
+
+def check_instance(oracle, prob, dtype, g, b, *, iters=None, tol=None, warm=None, eta=0.999, scale=1.0):
+    """Assert parity of instance b.  Returns (worst relative error, replayed?)."""
+    iters = prob.iters if iters is None else iters
+    o = oracle_run(oracle, prob, dtype, b, iters=iters, tol=tol, warm=warm, eta=eta)
+    git = int(g["res"]["iters"][b])
+    replayed = False
+    if "acc_hist" in g:
+        ga = g["acc_hist"][b, :git]
+        n = min(git, o.iters)
+        diff = np.nonzero(ga[:n] != o.acc_hist[:n])[0]
+        if diff.size or git != o.iters:
+            i = int(diff[0]) if diff.size else n - 1
+            cprev = o.c_hist[i - 1] if i > 0 else 1.0
+            tolv = prob.tol if tol is None else tol
+            margin = abs(o.c_hist[i] / (eta * cprev) - 1.0) if eta > 0 else 1.0
+            if git != o.iters and not diff.size and tolv > 0:
+                margin = min(margin, abs(o.c_hist[min(git, o.iters) - 1] / tolv - 1.0))
+            assert margin < TAU[dtype], (
+                f"instance {b}: decision differs at iteration {i} with oracle margin {margin:.3e} "
+                f"(not a floating-point near-tie)")
+            o = oracle_run(oracle, prob, dtype, b, iters=git, tol=0.0, forced=ga, warm=warm, eta=eta)
+            replayed = True
+    assert git == o.iters, f"instance {b}: iterations {git} vs oracle {o.iters}"
+    worst = 0.0
+    names = ARRAYS + (("D", "DE") if prob.du_lo is not None else ())
+    for n in names:
+        err = relerr(g[n][b], getattr(o, n))
+        worst = max(worst, err)
+        assert err <= TOL[dtype] * scale, f"instance {b} array {n}: rel err {err:.3e} > {TOL[dtype] * scale:.1e}"
+    for n, ov in (("x", o.x), ("u", o.u), ("du", o.DU)):
+        err = relerr(g[n][b], ov)
+        assert err <= TOL[dtype] * scale, f"instance {b} output {n}: rel err {err:.3e}"
+    # c = rho * sum d_j^2 is a sum of squared DIFFERENCES of O(S) iterates: each d_j carries an absolute
+    # rounding error <= u*S, so |delta c| <= 2 sqrt(rho c n_terms) u S on top of the relative bar
+    # (matters only once c has fallen to rounding level, e.g. converged tiny problems).
+    S = max(1.0, max(float(np.max(np.abs(getattr(o, n)))) for n in ("Z", "V", "TH", "BE", "LA", "X")))
+    u = 8 * (2.2e-16 if dtype == "f64" else 6e-8)
+    nterms = 8 * prob.N * prob.nb
+    floor = lambda c: 2.0 * np.sqrt(prob.rho * np.abs(c) * nterms) * u * S + 1e-300
+    assert abs(g["res"]["c"][b] - o.c_last) <= TOL_C[dtype] * abs(o.c_last) + floor(o.c_last), (
+        f"instance {b}: c {g['res']['c'][b]} vs {o.c_last}")
+    if "c_hist" in g:
+        gc = g["c_hist"][b, :git]
+        assert np.all(np.abs(gc - o.c_hist) <= TOL_C[dtype] * np.abs(o.c_hist) + floor(o.c_hist)), f"instance {b}: c history"
+    assert int(g["res"]["restarts"][b]) == o.restarts
+    return worst, replayed
+
+
+def check(oracle, pimpc, prob, dtype, *, engine="auto", instances=None, iters=None, tol=None, eta=0.999,
+          scale=1.0):
+    g = gpu_run(pimpc, prob, dtype, engine=engine, iters=iters, tol=tol, eta=eta)
+    inst = range(prob.batch) if instances is None else instances
+    worst, nrep = 0.0, 0
+    for b in inst:
+        w, r = check_instance(oracle, prob, dtype, g, b, iters=iters, tol=tol, eta=eta, scale=scale)
+        worst = max(worst, w); nrep += int(r)
+    return g, worst, nrep
+
+
+def check_properties(prob, dtype, g):
+    """Properties that hold at any size (used where the oracle cannot run every instance):
+    bound feasibility of the projected copies (exact), beta + lambda = 0,
+    the normal-cone condition of the z-update (14c), finite values, iteration counts."""
+    eps = 1e-12 if dtype == "f64" else 2e-5
+    lo = prob.lo.astype(g["Z"].dtype); hi = prob.hi.astype(g["Z"].dtype)
+    assert np.all(np.isfinite(g["Z"])) and np.all(np.isfinite(g["TH"]))
+    assert np.all(g["Z"] >= lo) and np.all(g["Z"] <= hi)
+    sc = max(1.0, float(np.max(np.abs(g["BE"]))))
+    assert float(np.max(np.abs(g["BE"].astype(np.float64) + g["LA"]))) <= eps * sc * 10
+    if prob.du_lo is not None:
+        assert np.all(g["D"] >= prob.du_lo.astype(g["D"].dtype)) and np.all(g["D"] <= prob.du_hi.astype(g["D"].dtype))
+    Zd = g["Z"].astype(np.float64)
+    t = 0.5
+    fix = np.clip(Zd + t * (g["TH"].astype(np.float64) - g["LA"]), prob.lo, prob.hi)
+    sc = max(1.0, float(np.max(np.abs(g["TH"]))))
+    assert float(np.max(np.abs(fix - Zd))) <= eps * sc * 100
+    np.testing.assert_array_equal(g["x"], g["Z"][..., :prob.nx])
+    np.testing.assert_array_equal(g["u"], g["Z"][..., prob.nx:])
