@@ -78,6 +78,9 @@ typedef struct {
     int sm_count;             /* SMs of the device                                                    */
     int grid, block;          /* launch shape of the iteration kernel of the last solve               */
     size_t smem_bytes;        /* dynamic shared memory of that kernel                                 */
+    double setup_ms;          /* device time of the cache kernel of the last solve (0 if it did not run) */
+    double iter_ms;           /* device time of the iteration kernel(s) of the last solve (CUDA events on
+                                 the handle's stream; pimpc_get_info waits for them)                  */
 } pimpc_info;
 
 const char *pimpc_version(void);
@@ -157,6 +160,8 @@ int pimpc_reset(pimpc_t h);
 /* Wait for the handle's stream; returns a deferred device-side error if one was raised. */
 int pimpc_sync(pimpc_t h);
 
+/* Launch shape, launch counts and device timings of the last solve.  Synchronises the stream if a
+ * solve is pending (the timings come from CUDA events recorded around the kernels). */
 int pimpc_get_info(pimpc_t h, pimpc_info *info);
 const char *pimpc_last_error(pimpc_t h);
 

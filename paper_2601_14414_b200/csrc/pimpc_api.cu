@@ -227,6 +227,8 @@ int pimpc_create(pimpc_t *out, int nx, int nu, int N, int batch, const pimpc_opt
     if (rc == PIMPC_OK) rc = launch_zero_state(h) < 0 ? PIMPC_ECUDA : PIMPC_OK;
     if (rc != PIMPC_OK) { std::string m = h->errmsg; pimpc_destroy(h); return fail(nullptr, rc, m); }
     h->info.sm_count = h->sm_count;
+    for (auto &e : h->ev)
+        if (cudaEventCreate(&e) != cudaSuccess) { pimpc_destroy(h); return fail(nullptr, PIMPC_ECUDA, "cudaEventCreate failed"); }
     *out = h;
     return PIMPC_OK;
 }
@@ -239,6 +241,7 @@ int pimpc_destroy(pimpc_t h)
                     h->H, h->M, h->S, h->X, h->DU, h->ctl, h->partial, h->hist_c, h->hist_a, h->err,
                     h->hat, h->W, h->G, h->rhs, h->blob};
     for (void *p : ptrs) if (p) cudaFree(p);
+    for (auto &e : h->ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();
     delete h;
     return PIMPC_OK;
@@ -367,6 +370,8 @@ int pimpc_solve(pimpc_t h, int max_iters, double tol)
     if (max_iters < 0) return fail(h, PIMPC_EINVAL, "max_iters < 0");
     if (h->hist_cap > 0 && max_iters > h->hist_cap) return fail(h, PIMPC_EINVAL, "max_iters exceeds opts.history");
     int launches = 0, n;
+    PIMPC_CUDA_TRY(h, cudaEventRecord(h->ev[0], h->stream));
+    h->ev_setup = h->cache_dirty;
     if (h->cache_dirty) {
         n = launch_setup(h); if (n < 0) return n;
         launches += n;
@@ -375,6 +380,7 @@ int pimpc_solve(pimpc_t h, int max_iters, double tol)
     }
     n = launch_begin(h); if (n < 0) return n;
     launches += n;
+    PIMPC_CUDA_TRY(h, cudaEventRecord(h->ev[1], h->stream));
 
     int engine = h->engine_req;
     std::string why;
@@ -389,6 +395,8 @@ int pimpc_solve(pimpc_t h, int max_iters, double tol)
         if (n < 0) return n;
         launches += n;
     }
+    PIMPC_CUDA_TRY(h, cudaEventRecord(h->ev[2], h->stream));
+    h->ev_pending = true;
     h->info.engine = engine;
     h->info.launches = launches;
     h->info.total_launches += launches;
@@ -510,6 +518,15 @@ int pimpc_sync(pimpc_t h)
 int pimpc_get_info(pimpc_t h, pimpc_info *info)
 {
     if (!h || !info) return fail(h, PIMPC_EINVAL, "null argument");
+    if (h->ev_pending && !h->poisoned) {
+        PIMPC_CUDA_TRY(h, cudaEventSynchronize(h->ev[2]));
+        float a = 0.f, b = 0.f;
+        PIMPC_CUDA_TRY(h, cudaEventElapsedTime(&a, h->ev[0], h->ev[1]));
+        PIMPC_CUDA_TRY(h, cudaEventElapsedTime(&b, h->ev[1], h->ev[2]));
+        h->info.setup_ms = h->ev_setup ? a : 0.0;
+        h->info.iter_ms = b;
+        h->ev_pending = false;
+    }
     h->info.device_bytes = h->device_bytes;
     h->info.sm_count = h->sm_count;
     *info = h->info;

@@ -89,6 +89,9 @@ struct pimpc_s {
     size_t blob_stride = 0;
     bool blob_dirty = true;
 
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // before cache kernel, before iteration, after iteration
+    bool ev_pending = false, ev_setup = false;
+
     bool cache_dirty = true;
     size_t device_bytes = 0;
     pimpc_info info{};

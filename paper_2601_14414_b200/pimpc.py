@@ -42,7 +42,8 @@ class pimpc_result(ctypes.Structure):
 class pimpc_info(ctypes.Structure):
     _fields_ = [("engine", ctypes.c_int), ("launches", ctypes.c_int), ("total_launches", ctypes.c_longlong),
                 ("device_bytes", ctypes.c_size_t), ("sm_count", ctypes.c_int), ("grid", ctypes.c_int),
-                ("block", ctypes.c_int), ("smem_bytes", ctypes.c_size_t)]
+                ("block", ctypes.c_int), ("smem_bytes", ctypes.c_size_t), ("setup_ms", ctypes.c_double),
+                ("iter_ms", ctypes.c_double)]
 
 
 RESULT_DTYPE = np.dtype([("c", "f8"), ("alpha", "f8"), ("iters", "i4"), ("restarts", "i4"),
