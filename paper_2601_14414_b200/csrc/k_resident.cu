@@ -1,14 +1,410 @@
-// RESIDENT engine placeholder (replaced by the register-resident persistent kernel).
+// RESIDENT engine: Algorithm 1 with one CTA per MPC instance and ONE launch per
+// solve.  Everything an instance needs for all its iterations stays on chip:
+//   * the stage matrices (rows of H_k, columns of Abar_{k+1}, rows of [A_k B_k], columns of B_k,
+//     rows of M_k) live in REGISTERS of the lane that owns the row -- they are read from HBM once
+//     per solve;
+//   * the iterates (z, v, theta, beta, lambda, d, delta; current and previous) live in registers
+//     of the same lane; the hats of steps 6/7 are recomputed from (cur, prev, kappa);
+//   * only the vectors a mat-vec needs from other lanes (w, v-beta, h, xbar, rhs, du) go through
+//     shared memory, read back with 16-byte broadcast loads.
+// Mapping: a group of LPS = pow2(ceil(nb/R)) lanes owns one stage, lane li owns rows li*R..li*R+R-1
+// of that stage; a warp owns 32/LPS consecutive stages; the CTA owns the whole horizon, so the
+// neighbour coupling (stage k needs w_{k+1} and xbar_k) and the reduction of c (step 4) cost three
+// CTA barriers per iteration and no global memory traffic.  The CTA loops over instances
+// (grid-stride), so a launch covers any batch.
+// c is reduced in a fixed order (xor butterflies; every warp repeats the second level), so every
+// thread takes the same accept/restart decision (steps 5-7) from bit-identical numbers.
+#include <algorithm>
+
 #include "pimpc_internal.h"
 
-bool resident_supported(const pimpc_s *, std::string *why)
+namespace {
+
+constexpr int pow2ceil_c(int v) { int p = 1; while (p < v) p <<= 1; return p; }
+
+__device__ __forceinline__ void ld4(const float *p, float (&o)[4])
 {
-    if (why) *why = "not built yet";
+    const float4 v = *reinterpret_cast<const float4 *>(p);
+    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void ld4(const double *p, double (&o)[4])
+{
+    const double2 a = *reinterpret_cast<const double2 *>(p), b = *reinterpret_cast<const double2 *>(p + 2);
+    o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
+}
+template <typename T> __device__ __forceinline__ T clipv(T v, T lo, T hi) { return fmin(fmax(v, lo), hi); }
+
+// alpha_j and kappa_j after j consecutive accepted steps from alpha_0 = 1:
+// alpha_{j+1} = 0.5 + 0.5 sqrt(1 + 4 alpha_j^2), kappa_j = (alpha_j - 1) / alpha_{j+1}.
+__global__ void k_alpha_table(double *alpha, double *kappa, int n)
+{
+    if (blockIdx.x || threadIdx.x) return;
+    double a = 1.0;
+    for (int j = 0; j < n; ++j) {
+        const double an = 0.5 + 0.5 * sqrt(1.0 + 4.0 * a * a);
+        alpha[j] = a;
+        kappa[j] = (a - 1.0) / an;
+        a = an;
+    }
+}
+
+template <typename T, int NX, int NU, int R>
+struct RCfg {
+    static constexpr int NB = NX + NU;
+    static constexpr int LPS = pow2ceil_c((NB + R - 1) / R);   // lanes per stage
+    static constexpr int SPW = 32 / LPS;                       // stages per warp
+    static constexpr int ROWP = LPS * R;                       // padded vector length of a stage
+    static constexpr int NBP = (NB + 3) / 4 * 4;
+    static constexpr int NUP = (NU + 3) / 4 * 4;
+    static constexpr int KAPN = 1024;                          // kappa table entries cached in smem
+    // Shared memory: one block per stage slot s = k+1 (slot 0 holds xbar_0, slot NS+1 a zero w), so every
+    // access of a lane is (one of three per-thread base registers) + a compile-time offset:
+    //   W  w_k = zhat - vhat - ebar + lambdahat      X  xbar_{k+1}        D  vhat - betahat     H  h_k
+    //   RH rhs of the Delta-u update    DU Delta u_k   AT columns of Abar_{k+1} (rows < nx), [R][NX/4][LPS][4]
+    static constexpr int OW = 0, OX = ROWP, OD = 2 * ROWP, OH = 3 * ROWP, ORH = 4 * ROWP, ODU = ORH + NUP,
+                         OAT = ODU + NUP, SS0 = OAT + NX * ROWP;
+    // stage stride == LPS (mod 32 words): the groups of a warp hit disjoint banks on own-element accesses
+    static constexpr int SS = SS0 + ((LPS - SS0 % 32) + 32) % 32;
+    static_assert(NX % 4 == 0, "RESIDENT engine needs nx % 4 == 0");
+    static_assert(NX % R == 0 && LPS <= 32 && LPS >= 4 && ROWP >= NBP && ROWP % 4 == 0 && SS % 4 == 0, "bad row blocking");
+    static size_t smem_bytes(int nwarps)
+    {
+        const size_t NS = (size_t)nwarps * SPW;
+        return ((NS + 2) * SS + KAPN) * sizeof(T) + 34 * sizeof(double);
+    }
+};
+
+template <typename T, int R>
+struct RState { T z[R], v[R], th[R], be[R], la[R], d[R], de[R]; };
+
+template <typename T, int NX, int NU, int R, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1)      // the register file is split per SM sub-partition: 7 warps x 72 regs
+k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__restrict__ kappa_tab, const int iters)
+{
+    using C = RCfg<T, NX, NU, R>;
+    constexpr int NB = C::NB, LPS = C::LPS, SPW = C::SPW, NBP = C::NBP, NUP = C::NUP, SS = C::SS;
+    constexpr int OW = C::OW, OX = C::OX, OD = C::OD, OH = C::OH, ORH = C::ORH, ODU = C::ODU, OAT = C::OAT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int NS = nwarps * SPW, N = p.N;
+    double *red = reinterpret_cast<double *>(smem_raw);       // [32] warp partials of c, [33] c of the last iteration
+    T *sKap = reinterpret_cast<T *>(red + 34);                // [KAPN]
+    T *sBlk = sKap + C::KAPN;                                 // [NS+2][SS]
+
+    const int li = lane % LPS, k = warp * SPW + lane / LPS;
+    const bool stage_ok = k < N;
+    const T rho = (T)p.rho;
+    T *const blk = sBlk + (size_t)(k + 1) * SS;               // block of the own stage
+    T *const own = blk + li * R;                              // + own rows
+    T *const atp = blk + OAT + li * 4;                        // + own lane slot of the Abar^T columns
+
+    for (int i = tid; i < (NS + 2) * SS; i += blockDim.x) sBlk[i] = (T)0;      // pads must stay finite zeros
+    for (int i = tid; i < min(iters + 1, C::KAPN); i += blockDim.x) sKap[i] = (T)kappa_tab[i];
+    __syncthreads();
+
+    for (int b = blockIdx.x; b < p.batch; b += gridDim.x) {
+        const InstCtl ctl0 = p.ctl[b];
+        const size_t sk = (size_t)b * N + (stage_ok ? k : 0);
+        // ---- stage matrices -> registers / smem (once per solve) ------------------------------
+        T Hrow[R][NBP], U[R][NBP], qv[R], ev[R], lo[R], hi[R], dlo[R], dhi[R];
+        bool isx[R], isu[R], isui[R];
+        RState<T, R> sa, sb;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int i = li * R + r;
+            const bool ok = stage_ok && i < NB;
+            isx[r] = ok && i < NX;
+            isu[r] = ok && i >= NX;
+            const bool inner = ok && k < N - 1;
+            isui[r] = isu[r] && inner;
+            const T *Hk = p.H + sk * NB * NB + (size_t)(ok ? i : 0) * NB;
+#pragma unroll
+            for (int j = 0; j < NBP; ++j) Hrow[r][j] = (ok && j < NB) ? Hk[j] : (T)0;
+            const T *A1 = p.A + (sk + (inner ? 1 : 0)) * NX * NX, *B1 = p.B + (sk + (inner ? 1 : 0)) * NX * NU;
+#pragma unroll
+            for (int q = 0; q < NX; ++q)                       // column i of Abar_{k+1} (rows < nx)
+                atp[((r * (NX / 4) + q / 4) * LPS) * 4 + (q & 3)] =
+                    !inner ? (T)0 : (i < NX ? A1[q * NX + i] : B1[q * NU + (i - NX)]);
+            const T *Ak = p.A + sk * NX * NX, *Bk = p.B + sk * NX * NU, *Mk = p.M + sk * NU * NU;
+#pragma unroll
+            for (int j = 0; j < NBP; ++j) {
+                T v = (T)0;
+                if (isx[r]) v = j < NX ? Ak[i * NX + j] : (j < NB ? Bk[i * NU + (j - NX)] : (T)0);    // row i of [A_k B_k]
+                else if (isu[r]) v = j < NX ? Bk[j * NU + (i - NX)] : (j < NB ? Mk[(i - NX) * NU + (j - NX)] : (T)0);
+                U[r][j] = v;                                   // u-rows: column of B_k, then row of M_k
+            }
+            qv[r] = ok ? p.qbar[(size_t)b * p.qbar_stride + i] : (T)0;
+            ev[r] = (isx[r] && p.e) ? p.e[sk * NX + i] : (T)0;
+            lo[r] = ok ? p.lo[(size_t)b * p.bnd_stride + i] : (T)0;
+            hi[r] = ok ? p.hi[(size_t)b * p.bnd_stride + i] : (T)0;
+            dlo[r] = (isu[r] && p.has_du) ? p.dlo[(size_t)b * p.dbnd_stride + (i - NX)] : (T)0;
+            dhi[r] = (isu[r] && p.has_du) ? p.dhi[(size_t)b * p.dbnd_stride + (i - NX)] : (T)0;
+            // ---- iterate of the previous solve / cold start (hats = iterates: prev = cur) --------
+            const T *rec = p.S + (size_t)ctl0.i_cur * p.buf_stride + p.st(b, stage_ok ? k : 0);
+            sa.z[r] = ok ? rec[p.oZ() + i] : (T)0;
+            sa.v[r] = ok ? rec[p.oV() + i] : (T)0;
+            sa.th[r] = ok ? rec[p.oTH() + i] : (T)0;
+            sa.be[r] = ok ? rec[p.oBE() + i] : (T)0;
+            sa.la[r] = ok ? rec[p.oLA() + i] : (T)0;
+            sa.d[r] = (isu[r] && p.has_du) ? rec[p.oD() + (i - NX)] : (T)0;
+            sa.de[r] = (isu[r] && p.has_du) ? rec[p.oDE() + (i - NX)] : (T)0;
+        }
+        sb = sa;
+        if (tid < C::ROWP)                                     // slot 0: xbar_0 = (x(t); u(t-1))
+            sBlk[OX + tid] = tid < NX ? p.x0[(size_t)b * NX + tid] : (tid < NB ? p.uprev[(size_t)b * NU + (tid - NX)] : (T)0);
+
+        T kap = (T)0;
+        double c_prev = p.c0;
+        int jacc = 0, restarts = 0, it_done = 0;
+        bool done = false;
+        const bool has_du = p.has_du != 0;
+        if (tid == 0) red[33] = p.c0;
+
+        // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.
+        auto iteration = [&](RState<T, R> &cur, RState<T, R> &prv, const int it) -> bool {
+            T zh[R], vh[R], thh[R], beh[R], lah[R], dh[R], deh[R], dv[R];
+            // steps 6/7 of the previous iteration: hats from (cur, prev, kappa)
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                zh[r] = cur.z[r] + kap * (cur.z[r] - prv.z[r]);
+                vh[r] = cur.v[r] + kap * (cur.v[r] - prv.v[r]);
+                thh[r] = cur.th[r] + kap * (cur.th[r] - prv.th[r]);
+                beh[r] = cur.be[r] + kap * (cur.be[r] - prv.be[r]);
+                lah[r] = cur.la[r] + kap * (cur.la[r] - prv.la[r]);
+                dh[r] = cur.d[r] + kap * (cur.d[r] - prv.d[r]);
+                deh[r] = cur.de[r] + kap * (cur.de[r] - prv.de[r]);
+                dv[r] = vh[r] - beh[r];
+                own[OW + r] = zh[r] - vh[r] - ev[r] + lah[r];
+                own[OD + r] = dv[r];
+            }
+            __syncthreads();
+            // step 1: g = Abar_{k+1}^T w_{k+1}, rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat]
+            T g[R], rd[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) { g[r] = (T)0; rd[r] = (T)0; }
+#pragma unroll
+            for (int c4 = 0; c4 < NX; c4 += 4) {
+                T w4[4], d4[4];
+                ld4(blk + SS + OW + c4, w4);
+                ld4(blk + OD + c4, d4);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    T a4[4];
+                    ld4(atp + ((r * (NX / 4) + c4 / 4) * LPS) * 4, a4);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) { g[r] += a4[q] * w4[q]; rd[r] += U[r][c4 + q] * d4[q]; }
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (isui[r]) g[r] += own[SS + OW + r];                             // the [0 I] rows of Abar_{k+1}
+                own[OH + r] = qv[r] + rho * (zh[r] - thh[r]) + rho * g[r];        // h_k (index reading R2)
+                if (isu[r]) own[ORH - NX + r] = rd[r] + dv[r] + (dh[r] - deh[r]);
+            }
+            __syncwarp();
+            T x[R], du[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) { x[r] = (T)0; du[r] = (T)0; }
+#pragma unroll
+            for (int c4 = 0; c4 < NBP; c4 += 4) {
+                T h4[4];
+                ld4(blk + OH + c4, h4);
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) x[r] += Hrow[r][c4 + q] * h4[q];          // xbar_{k+1} = H_k h_k
+            }
+#pragma unroll
+            for (int c4 = 0; c4 < NUP; c4 += 4) {
+                T r4[4];
+                ld4(blk + ORH + c4, r4);
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) if (NX + c4 + q < NBP) du[r] += U[r][NX + c4 + q] * r4[q];   // Delta u_k = M_k rhs (u-rows)
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                own[OX + r] = x[r];
+                if (isu[r]) own[ODU - NX + r] = du[r];
+            }
+            __syncthreads();
+            // steps 2-4
+            T dot[R], avx[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) { dot[r] = (T)0; avx[r] = (T)0; }
+#pragma unroll
+            for (int c4 = 0; c4 < NBP; c4 += 4) {
+                T x4[4];
+                ld4(blk - SS + OX + c4, x4);
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) dot[r] += U[r][c4 + q] * x4[q];           // [A_k B_k] xbar_k (x-rows)
+            }
+#pragma unroll
+            for (int c4 = 0; c4 < NUP; c4 += 4) {
+                T u4[4];
+                ld4(blk + ODU + c4, u4);
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) if (NX + c4 + q < NBP) avx[r] += U[r][NX + c4 + q] * u4[q];  // B_k Delta u_k (x-rows)
+            }
+            T acc = (T)0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const T xpi = own[-SS + OX + r];
+                const T av = (isx[r] ? avx[r] : du[r]) + beh[r];                 // a = Bbar du + betahat
+                const T bv = (isx[r] ? dot[r] + ev[r] : xpi) - lah[r];           // b = Abar xbar_k + ebar - lambdahat
+                const T gam = av - bv;
+                const T zn = clipv(((T)2 * (x[r] + thh[r] + bv) + gam) * (T)(1.0 / 3.0), lo[r], hi[r]);
+                const T vn = (T)0.5 * (zn + gam);
+                const T thn = thh[r] + x[r] - zn;
+                const T ben = av - vn;
+                const T lan = zn - bv - vn;
+                const T d0 = thn - thh[r], d1 = ben - beh[r], d2 = lan - lah[r], d3 = zn - zh[r], d4 = vn - vh[r];
+                const T d5 = (zn - vn) - (zh[r] - vh[r]);
+                T a = d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
+                const T dn = clipv(du[r] + deh[r], dlo[r], dhi[r]);             // Delta-u box copy (reading R12), u-rows
+                const T den = deh[r] + du[r] - dn;
+                const T e0 = den - deh[r], e1 = dn - dh[r];
+                if (has_du && isu[r]) { a += e0 * e0 + e1 * e1; prv.d[r] = dn; prv.de[r] = den; }
+                if (isx[r] || isu[r]) { acc += a; prv.z[r] = zn; prv.v[r] = vn; prv.th[r] = thn; prv.be[r] = ben; prv.la[r] = lan; }
+            }
+            // step 4: c = rho * sum (fixed order: group butterfly in T, then double)
+#pragma unroll
+            for (int o = LPS / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            double s = (double)acc;
+#pragma unroll
+            for (int o = 16; o >= LPS; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) red[warp] = s;
+            __syncthreads();
+            s = lane < nwarps ? red[lane] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            // steps 5-7; every thread decides from the same bits
+            const double c = p.rho * s;
+            if (tid == 0) red[33] = c;
+            it_done = it + 1;
+            const bool stop = p.tol > 0.0 && c < p.tol;
+            const bool accept = !stop && c <= p.eta * c_prev;
+            if (tid == 0 && p.hist_c && it < p.hist_cap) {
+                p.hist_c[(size_t)b * p.hist_cap + it] = c;
+                p.hist_a[(size_t)b * p.hist_cap + it] = (unsigned char)accept;
+            }
+            if (stop) { done = true; return true; }
+            if (accept) {
+                kap = jacc < C::KAPN ? sKap[jacc] : (T)kappa_tab[jacc];
+                ++jacc;
+            } else {
+                kap = (T)0; jacc = 0; ++restarts;
+            }
+            c_prev = c;
+            return false;
+        };
+
+        __syncthreads();
+        bool in_b = false;                       // which of (sa, sb) holds the current iterate
+        for (int it = 0; it < iters; it += 2) {
+            if (iteration(sa, sb, it)) { in_b = true; break; }
+            in_b = true;
+            if (it + 1 >= iters) break;
+            if (iteration(sb, sa, it + 1)) { in_b = false; break; }
+            in_b = false;
+        }
+        if (in_b) sa = sb;                       // register moves; a reference select would force local memory
+        const RState<T, R> &fin = sa;
+
+        // ---- results: iterate -> S[i_cur], xbar and Delta u of the last iteration, control block ----
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int i = li * R + r;
+            if (isx[r] || isu[r]) {
+                T *rec = p.S + (size_t)ctl0.i_cur * p.buf_stride + p.st(b, k);
+                rec[p.oZ() + i] = fin.z[r]; rec[p.oV() + i] = fin.v[r]; rec[p.oTH() + i] = fin.th[r];
+                rec[p.oBE() + i] = fin.be[r]; rec[p.oLA() + i] = fin.la[r];
+                p.X[sk * NB + i] = own[OX + r];
+                if (isu[r]) {
+                    p.DU[sk * NU + (i - NX)] = own[ODU - NX + r];
+                    if (has_du) { rec[p.oD() + (i - NX)] = fin.d[r]; rec[p.oDE() + (i - NX)] = fin.de[r]; }
+                }
+            }
+        }
+        if (tid == 0) {
+            InstCtl c = ctl0;
+            c.alpha = alpha_tab[jacc]; c.c_prev = c_prev; c.c_last = red[33]; c.kappa = (double)kap;
+            c.done = done ? 1 : 0; c.iters = it_done; c.restarts = restarts;
+            p.ctl[b] = c;
+        }
+        __syncthreads();
+    }
+}
+
+template <typename T, int NX, int NU, int R, int MAXT>
+int launch_resident(pimpc_s *h, int iters, double tol, int nwarps)
+{
+    using C = RCfg<T, NX, NU, R>;
+    auto kern = k_resident<T, NX, NU, R, MAXT>;
+    const size_t smem = C::smem_bytes(nwarps);
+    PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    PIMPC_CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nwarps * 32, smem));
+    if (occ < 1) { h->errmsg = "RESIDENT kernel does not fit on an SM"; return PIMPC_EINVAL; }
+    const int grid = std::min(h->batch, h->sm_count * occ);
+    Prob<T> p = make_prob<T>(h, tol);
+    kern<<<grid, nwarps * 32, smem, h->stream>>>(p, h->alpha_tab, h->kappa_tab, iters);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    h->info.grid = grid; h->info.block = nwarps * 32; h->info.smem_bytes = smem;
+    return 1;
+}
+
+// instantiation table: (dtype, nx, nu) -> rows per lane, stages per warp, thread ceilings
+struct ResidentPlan { int spw; int max_stages; };
+
+bool plan_for(const pimpc_s *h, ResidentPlan *pl)
+{
+    if (h->dtype == PIMPC_F32 && h->nx == 12 && h->nu == 4) { *pl = {2, 64}; return true; }
+    if (h->dtype == PIMPC_F64 && h->nx == 4 && h->nu == 2) { *pl = {4, 64}; return true; }
+    if (h->dtype == PIMPC_F32 && h->nx == 4 && h->nu == 2) { *pl = {4, 128}; return true; }
     return false;
 }
 
-int run_resident(pimpc_s *h, int, double)
+} // namespace
+
+bool resident_supported(const pimpc_s *h, std::string *why)
 {
-    h->errmsg = "RESIDENT engine not available";
-    return PIMPC_EINVAL;
+    ResidentPlan pl;
+    if (!plan_for(h, &pl)) { if (why) *why = "no register-resident instantiation for this (dtype, nx, nu)"; return false; }
+    if (h->N > pl.max_stages) { if (why) *why = "horizon exceeds what one CTA keeps in registers"; return false; }
+    return true;
+}
+
+int run_resident(pimpc_s *h, int iters, double tol)
+{
+    ResidentPlan pl;
+    if (!plan_for(h, &pl) || h->N > pl.max_stages) { h->errmsg = "RESIDENT engine not applicable"; return PIMPC_EINVAL; }
+    int launches = 0;
+    if (h->tab_cap < iters + 2) {
+        if (h->alpha_tab) { cudaFree(h->alpha_tab); cudaFree(h->kappa_tab); h->alpha_tab = h->kappa_tab = nullptr; }
+        const int cap = std::max(iters + 2, 1024);
+        PIMPC_CUDA_TRY(h, cudaMalloc(&h->alpha_tab, cap * sizeof(double)));
+        PIMPC_CUDA_TRY(h, cudaMalloc(&h->kappa_tab, cap * sizeof(double)));
+        h->device_bytes += 2 * (size_t)cap * sizeof(double);
+        k_alpha_table<<<1, 32, 0, h->stream>>>(h->alpha_tab, h->kappa_tab, cap);
+        PIMPC_CUDA_TRY(h, cudaGetLastError());
+        h->tab_cap = cap;
+        ++launches;
+    }
+    const int nwarps = (h->N + pl.spw - 1) / pl.spw;
+    int n;
+    if (h->dtype == PIMPC_F32 && h->nx == 12) {
+        n = nwarps <= 25 ? launch_resident<float, 12, 4, 1, 800>(h, iters, tol, nwarps)
+                         : launch_resident<float, 12, 4, 1, 1024>(h, iters, tol, nwarps);
+    } else if (h->dtype == PIMPC_F64) {
+        n = launch_resident<double, 4, 2, 1, 512>(h, iters, tol, nwarps);
+    } else {
+        n = launch_resident<float, 4, 2, 1, 1024>(h, iters, tol, nwarps);
+    }
+    return n < 0 ? n : n + launches;
 }

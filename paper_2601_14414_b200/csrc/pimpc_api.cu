@@ -239,7 +239,7 @@ int pimpc_destroy(pimpc_t h)
     if (!h->poisoned) cudaStreamSynchronize(h->stream);
     void *ptrs[] = {h->A, h->B, h->e, h->x0, h->uprev, h->Q, h->R, h->P, h->Wdu, h->qbar, h->lo, h->hi, h->dlo, h->dhi,
                     h->H, h->M, h->S, h->X, h->DU, h->ctl, h->partial, h->hist_c, h->hist_a, h->err,
-                    h->hat, h->W, h->G, h->rhs, h->blob};
+                    h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (auto &e : h->ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();

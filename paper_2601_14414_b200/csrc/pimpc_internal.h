@@ -84,6 +84,9 @@ struct pimpc_s {
     int *err = nullptr;
     // scratch of the STAGED engine (allocated on first use)
     void *hat = nullptr, *W = nullptr, *G = nullptr, *rhs = nullptr;
+    // alpha_j / kappa_j tables of the fused engines (j consecutive accepted steps), [tab_cap] doubles
+    double *alpha_tab = nullptr, *kappa_tab = nullptr;
+    int tab_cap = 0;
     // engine-private storage (packed blobs of the STREAM engine etc.)
     void *blob = nullptr;
     size_t blob_stride = 0;

@@ -3,8 +3,9 @@
 Protocol (SURVEY.md section 8(c) P-flip):
   * both sides log (c^{i+1}, accept bit) per iteration and instance;
   * identical decision sequences -> compare every iterate array element by element;
-  * if they first differ at i*, the oracle's margin |c/(eta c_prev) - 1| at i* must be below
-    tau (1e-11 fp64, 1e-5 fp32), i.e. a genuine floating-point near-tie -- otherwise FAIL --
+  * if they first differ at i*, the oracle's own gap |c - eta c_prev| at i* must be below
+    tau * eta c_prev (tau = 1e-11 fp64, 1e-5 fp32) plus the absolute rounding floor of the two
+    residuals, i.e. a genuine floating-point near-tie -- otherwise FAIL --
     and the oracle is re-run with the GPU's decision sequence forced (never the other way round);
   * fp32 runs: the oracle is fed the fp32-rounded inputs promoted to double.
 Metric: per array and instance  max|g - o| / max(max|o|, tiny)  <= 1e-9 (fp64) / 1e-4 (fp32);
@@ -65,20 +66,32 @@ def check_instance(oracle, prob, dtype, g, b, *, iters=None, tol=None, warm=None
     o = oracle_run(oracle, prob, dtype, b, iters=iters, tol=tol, warm=warm, eta=eta)
     git = int(g["res"]["iters"][b])
     replayed = False
+    # c = rho * sum d_j^2 is a sum of squared DIFFERENCES of O(S) iterates: each d_j carries an absolute
+    # rounding error <= u*S, so |delta c| <= 2 sqrt(rho c n_terms) u S + rho n_terms (u S)^2 on top of the relative bar
+    # (matters only once c has fallen to rounding level, e.g. converged tiny problems); DESIGN.md "Tolerances".
+    S = max(1.0, max(float(np.max(np.abs(getattr(o, n)))) for n in ("Z", "V", "TH", "BE", "LA", "X")))
+    u = 8 * (2.2e-16 if dtype == "f64" else 6e-8)
+    nterms = 8 * prob.N * prob.nb
+    floor = lambda c: 2.0 * np.sqrt(prob.rho * np.abs(c) * nterms) * u * S + prob.rho * nterms * (u * S) ** 2
     if "acc_hist" in g:
         ga = g["acc_hist"][b, :git]
         n = min(git, o.iters)
         diff = np.nonzero(ga[:n] != o.acc_hist[:n])[0]
         if diff.size or git != o.iters:
+            # a differing decision must be a floating-point near-tie of the ORACLE's own comparison:
+            # |c - eta c_prev| within tau (relative) plus the rounding floor of the two residuals
             i = int(diff[0]) if diff.size else n - 1
             cprev = o.c_hist[i - 1] if i > 0 else 1.0
             tolv = prob.tol if tol is None else tol
-            margin = abs(o.c_hist[i] / (eta * cprev) - 1.0) if eta > 0 else 1.0
+            gap = abs(o.c_hist[i] - eta * cprev) if eta > 0 else np.inf
+            slack = TAU[dtype] * eta * cprev + floor(o.c_hist[i]) + eta * floor(cprev)
             if git != o.iters and not diff.size and tolv > 0:
-                margin = min(margin, abs(o.c_hist[min(git, o.iters) - 1] / tolv - 1.0))
-            assert margin < TAU[dtype], (
-                f"instance {b}: decision differs at iteration {i} with oracle margin {margin:.3e} "
-                f"(not a floating-point near-tie)")
+                cl = o.c_hist[min(git, o.iters) - 1]
+                if abs(cl - tolv) <= TAU[dtype] * tolv + floor(cl):
+                    gap = 0.0
+            assert gap <= slack, (
+                f"instance {b}: decision differs at iteration {i}: oracle |c - eta c_prev| = {gap:.3e} > "
+                f"{slack:.3e} (not a floating-point near-tie)")
             o = oracle_run(oracle, prob, dtype, b, iters=git, tol=0.0, forced=ga, warm=warm, eta=eta)
             replayed = True
     assert git == o.iters, f"instance {b}: iterations {git} vs oracle {o.iters}"
@@ -91,13 +104,6 @@ def check_instance(oracle, prob, dtype, g, b, *, iters=None, tol=None, warm=None
     for n, ov in (("x", o.x), ("u", o.u), ("du", o.DU)):
         err = relerr(g[n][b], ov)
         assert err <= TOL[dtype] * scale, f"instance {b} output {n}: rel err {err:.3e}"
-    # c = rho * sum d_j^2 is a sum of squared DIFFERENCES of O(S) iterates: each d_j carries an absolute
-    # rounding error <= u*S, so |delta c| <= 2 sqrt(rho c n_terms) u S on top of the relative bar
-    # (matters only once c has fallen to rounding level, e.g. converged tiny problems).
-    S = max(1.0, max(float(np.max(np.abs(getattr(o, n)))) for n in ("Z", "V", "TH", "BE", "LA", "X")))
-    u = 8 * (2.2e-16 if dtype == "f64" else 6e-8)
-    nterms = 8 * prob.N * prob.nb
-    floor = lambda c: 2.0 * np.sqrt(prob.rho * np.abs(c) * nterms) * u * S + 1e-300
     assert abs(g["res"]["c"][b] - o.c_last) <= TOL_C[dtype] * abs(o.c_last) + floor(o.c_last), (
         f"instance {b}: c {g['res']['c'][b]} vs {o.c_last}")
     if "c_hist" in g:
