@@ -62,7 +62,7 @@ struct RCfg {
     //   W  w_k = zhat - vhat - ebar + lambdahat      X  xbar_{k+1}        D  vhat - betahat     H  h_k
     //   RH rhs of the Delta-u update    DU Delta u_k   AT columns of Abar_{k+1} (rows < nx), [R][NX/4][LPS][4]
     static constexpr int OW = 0, OX = ROWP, OD = 2 * ROWP, OH = 3 * ROWP, ORH = 4 * ROWP, ODU = ORH + NUP,
-                         OAT = ODU + NUP, SS0 = OAT + NX * ROWP;
+                         OC = ODU + NUP /* qbar, e, du_lo, du_hi rows */, OAT = OC + 4 * ROWP, SS0 = OAT + NX * ROWP;
     // stage stride == LPS (mod 32 words): the groups of a warp hit disjoint banks on own-element accesses
     static constexpr int SS = SS0 + ((LPS - SS0 % 32) + 32) % 32;
     static_assert(NX % 4 == 0, "RESIDENT engine needs nx % 4 == 0");
@@ -70,25 +70,28 @@ struct RCfg {
     static size_t smem_bytes(int nwarps)
     {
         const size_t NS = (size_t)nwarps * SPW;
-        return ((NS + 2) * SS + KAPN) * sizeof(T) + 34 * sizeof(double);
+        return ((NS + 2) * SS + KAPN) * sizeof(T) + 36 * sizeof(double);
     }
 };
 
 template <typename T, int R>
 struct RState { T z[R], v[R], th[R], be[R], la[R], d[R], de[R]; };
 
-template <typename T, int NX, int NU, int R, int MAXT>
+// DU: the Delta-u box block (reading R12) is active.  Pad rows / pad stages carry zero matrices, zero
+// bounds and zero iterates, so they run the same instructions and contribute exact zeros.
+template <typename T, int NX, int NU, int R, int MAXT, bool DU>
 __global__ void __launch_bounds__(MAXT, 1)      // the register file is split per SM sub-partition: 7 warps x 72 regs
 k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__restrict__ kappa_tab, const int iters)
 {
     using C = RCfg<T, NX, NU, R>;
     constexpr int NB = C::NB, LPS = C::LPS, SPW = C::SPW, NBP = C::NBP, NUP = C::NUP, SS = C::SS;
-    constexpr int OW = C::OW, OX = C::OX, OD = C::OD, OH = C::OH, ORH = C::ORH, ODU = C::ODU, OAT = C::OAT;
+    constexpr int OW = C::OW, OX = C::OX, OD = C::OD, OH = C::OH, ORH = C::ORH, ODU = C::ODU, OAT = C::OAT, OC = C::OC;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
     const int NS = nwarps * SPW, N = p.N;
-    double *red = reinterpret_cast<double *>(smem_raw);       // [32] warp partials of c, [33] c of the last iteration
-    T *sKap = reinterpret_cast<T *>(red + 34);                // [KAPN]
+    double *red = reinterpret_cast<double *>(smem_raw);       // [32] warp partials of c, [32..33] c of the last two iterations
+    int *sCnt = reinterpret_cast<int *>(red + 34);            // [0] restarts
+    T *sKap = reinterpret_cast<T *>(red + 36);                // [KAPN]
     T *sBlk = sKap + C::KAPN;                                 // [NS+2][SS]
 
     const int li = lane % LPS, k = warp * SPW + lane / LPS;
@@ -97,26 +100,26 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
     T *const blk = sBlk + (size_t)(k + 1) * SS;               // block of the own stage
     T *const own = blk + li * R;                              // + own rows
     T *const atp = blk + OAT + li * 4;                        // + own lane slot of the Abar^T columns
+    const bool has_e = p.e != nullptr, has_q = p.has_q != 0;
 
     for (int i = tid; i < (NS + 2) * SS; i += blockDim.x) sBlk[i] = (T)0;      // pads must stay finite zeros
     for (int i = tid; i < min(iters + 1, C::KAPN); i += blockDim.x) sKap[i] = (T)kappa_tab[i];
     __syncthreads();
 
     for (int b = blockIdx.x; b < p.batch; b += gridDim.x) {
-        const InstCtl ctl0 = p.ctl[b];
+        const int i_cur = p.ctl[b].i_cur;
         const size_t sk = (size_t)b * N + (stage_ok ? k : 0);
         // ---- stage matrices -> registers / smem (once per solve) ------------------------------
-        T Hrow[R][NBP], U[R][NBP], qv[R], ev[R], lo[R], hi[R], dlo[R], dhi[R];
-        bool isx[R], isu[R], isui[R];
+        T Hrow[R][NBP], U[R][NBP], lo[R], hi[R];
+        bool isx[R];
         RState<T, R> sa, sb;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int i = li * R + r;
             const bool ok = stage_ok && i < NB;
-            isx[r] = ok && i < NX;
-            isu[r] = ok && i >= NX;
+            isx[r] = i < NX || !stage_ok;              // pad stages: every row takes the (all-zero) x-row path
+            const bool okx = ok && i < NX, oku = ok && i >= NX;
             const bool inner = ok && k < N - 1;
-            isui[r] = isu[r] && inner;
             const T *Hk = p.H + sk * NB * NB + (size_t)(ok ? i : 0) * NB;
 #pragma unroll
             for (int j = 0; j < NBP; ++j) Hrow[r][j] = (ok && j < NB) ? Hk[j] : (T)0;
@@ -129,40 +132,42 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
             for (int j = 0; j < NBP; ++j) {
                 T v = (T)0;
-                if (isx[r]) v = j < NX ? Ak[i * NX + j] : (j < NB ? Bk[i * NU + (j - NX)] : (T)0);    // row i of [A_k B_k]
-                else if (isu[r]) v = j < NX ? Bk[j * NU + (i - NX)] : (j < NB ? Mk[(i - NX) * NU + (j - NX)] : (T)0);
+                if (okx) v = j < NX ? Ak[i * NX + j] : (j < NB ? Bk[i * NU + (j - NX)] : (T)0);    // row i of [A_k B_k]
+                else if (oku) v = j < NX ? Bk[j * NU + (i - NX)] : (j < NB ? Mk[(i - NX) * NU + (j - NX)] : (T)0);
                 U[r][j] = v;                                   // u-rows: column of B_k, then row of M_k
             }
-            qv[r] = ok ? p.qbar[(size_t)b * p.qbar_stride + i] : (T)0;
-            ev[r] = (isx[r] && p.e) ? p.e[sk * NX + i] : (T)0;
             lo[r] = ok ? p.lo[(size_t)b * p.bnd_stride + i] : (T)0;
             hi[r] = ok ? p.hi[(size_t)b * p.bnd_stride + i] : (T)0;
-            dlo[r] = (isu[r] && p.has_du) ? p.dlo[(size_t)b * p.dbnd_stride + (i - NX)] : (T)0;
-            dhi[r] = (isu[r] && p.has_du) ? p.dhi[(size_t)b * p.dbnd_stride + (i - NX)] : (T)0;
+            // per-row constants read back from smem only when present: qbar_i, e_i, du bounds
+            own[OC + r] = ok ? p.qbar[(size_t)b * p.qbar_stride + i] : (T)0;
+            own[OC + C::ROWP + r] = (okx && has_e) ? p.e[sk * NX + i] : (T)0;
+            own[OC + 2 * C::ROWP + r] = (oku && DU) ? p.dlo[(size_t)b * p.dbnd_stride + (i - NX)] : (T)0;
+            own[OC + 3 * C::ROWP + r] = (oku && DU) ? p.dhi[(size_t)b * p.dbnd_stride + (i - NX)] : (T)0;
             // ---- iterate of the previous solve / cold start (hats = iterates: prev = cur) --------
-            const T *rec = p.S + (size_t)ctl0.i_cur * p.buf_stride + p.st(b, stage_ok ? k : 0);
+            const T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(b, stage_ok ? k : 0);
             sa.z[r] = ok ? rec[p.oZ() + i] : (T)0;
             sa.v[r] = ok ? rec[p.oV() + i] : (T)0;
             sa.th[r] = ok ? rec[p.oTH() + i] : (T)0;
             sa.be[r] = ok ? rec[p.oBE() + i] : (T)0;
             sa.la[r] = ok ? rec[p.oLA() + i] : (T)0;
-            sa.d[r] = (isu[r] && p.has_du) ? rec[p.oD() + (i - NX)] : (T)0;
-            sa.de[r] = (isu[r] && p.has_du) ? rec[p.oDE() + (i - NX)] : (T)0;
+            sa.d[r] = (oku && DU) ? rec[p.oD() + (i - NX)] : (T)0;
+            sa.de[r] = (oku && DU) ? rec[p.oDE() + (i - NX)] : (T)0;
         }
         sb = sa;
         if (tid < C::ROWP)                                     // slot 0: xbar_0 = (x(t); u(t-1))
             sBlk[OX + tid] = tid < NX ? p.x0[(size_t)b * NX + tid] : (tid < NB ? p.uprev[(size_t)b * NU + (tid - NX)] : (T)0);
+        if (tid == 0) { red[32] = p.c0; red[33] = p.c0; sCnt[0] = 0; }
 
         T kap = (T)0;
-        double c_prev = p.c0;
-        int jacc = 0, restarts = 0, it_done = 0;
+        int jacc = 0, it_done = 0;
         bool done = false;
-        const bool has_du = p.has_du != 0;
-        if (tid == 0) red[33] = p.c0;
+        double *const hc = p.hist_c ? p.hist_c + (size_t)b * p.hist_cap : nullptr;
+        unsigned char *const ha = p.hist_a ? p.hist_a + (size_t)b * p.hist_cap : nullptr;
 
         // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.
-        auto iteration = [&](RState<T, R> &cur, RState<T, R> &prv, const int it) -> bool {
-            T zh[R], vh[R], thh[R], beh[R], lah[R], dh[R], deh[R], dv[R];
+        // par = it & 1 (compile-time after unrolling by two): c^{i} sits in red[32 + (par ^ 1)], c^{i+1} goes to red[32 + par].
+        auto iteration = [&](RState<T, R> &cur, RState<T, R> &prv, const int it, const int par) -> bool {
+            T zh[R], vh[R], thh[R], beh[R], lah[R], dh[R], deh[R], dv[R], ev[R];
             // steps 6/7 of the previous iteration: hats from (cur, prev, kappa)
 #pragma unroll
             for (int r = 0; r < R; ++r) {
@@ -171,17 +176,22 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 thh[r] = cur.th[r] + kap * (cur.th[r] - prv.th[r]);
                 beh[r] = cur.be[r] + kap * (cur.be[r] - prv.be[r]);
                 lah[r] = cur.la[r] + kap * (cur.la[r] - prv.la[r]);
-                dh[r] = cur.d[r] + kap * (cur.d[r] - prv.d[r]);
-                deh[r] = cur.de[r] + kap * (cur.de[r] - prv.de[r]);
+                if (DU) {
+                    dh[r] = cur.d[r] + kap * (cur.d[r] - prv.d[r]);
+                    deh[r] = cur.de[r] + kap * (cur.de[r] - prv.de[r]);
+                }
                 dv[r] = vh[r] - beh[r];
-                own[OW + r] = zh[r] - vh[r] - ev[r] + lah[r];
+                T w = zh[r] - vh[r] + lah[r];
+                ev[r] = (T)0;
+                if (has_e) { ev[r] = own[OC + C::ROWP + r]; w -= ev[r]; }
+                own[OW + r] = w;
                 own[OD + r] = dv[r];
             }
             __syncthreads();
             // step 1: g = Abar_{k+1}^T w_{k+1}, rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat]
-            T g[R], rd[R];
+            T g[R][2], rd[R][2];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { g[r] = (T)0; rd[r] = (T)0; }
+            for (int r = 0; r < R; ++r) { g[r][0] = g[r][1] = (T)0; rd[r][0] = rd[r][1] = (T)0; }
 #pragma unroll
             for (int c4 = 0; c4 < NX; c4 += 4) {
                 T w4[4], d4[4];
@@ -192,19 +202,24 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                     T a4[4];
                     ld4(atp + ((r * (NX / 4) + c4 / 4) * LPS) * 4, a4);
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) { g[r] += a4[q] * w4[q]; rd[r] += U[r][c4 + q] * d4[q]; }
+                    for (int q = 0; q < 4; ++q) { g[r][q & 1] += a4[q] * w4[q]; rd[r][q & 1] += U[r][c4 + q] * d4[q]; }
                 }
             }
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                if (isui[r]) g[r] += own[SS + OW + r];                             // the [0 I] rows of Abar_{k+1}
-                own[OH + r] = qv[r] + rho * (zh[r] - thh[r]) + rho * g[r];        // h_k (index reading R2)
-                if (isu[r]) own[ORH - NX + r] = rd[r] + dv[r] + (dh[r] - deh[r]);
+                T gg = g[r][0] + g[r][1];
+                if (!isx[r]) gg += own[SS + OW + r];                                // the [0 I] rows of Abar_{k+1}
+                T hh = rho * (zh[r] - thh[r]) + rho * gg;                           // h_k (index reading R2)
+                if (has_q) hh += own[OC + r];
+                own[OH + r] = hh;
+                T rr = rd[r][0] + rd[r][1] + dv[r];
+                if (DU) rr += dh[r] - deh[r];
+                if (!isx[r]) own[ORH - NX + r] = rr;
             }
             __syncwarp();
-            T x[R], du[R];
+            T x[R][2], du[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { x[r] = (T)0; du[r] = (T)0; }
+            for (int r = 0; r < R; ++r) { x[r][0] = x[r][1] = (T)0; du[r] = (T)0; }
 #pragma unroll
             for (int c4 = 0; c4 < NBP; c4 += 4) {
                 T h4[4];
@@ -212,7 +227,7 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) x[r] += Hrow[r][c4 + q] * h4[q];          // xbar_{k+1} = H_k h_k
+                    for (int q = 0; q < 4; ++q) x[r][q & 1] += Hrow[r][c4 + q] * h4[q];   // xbar_{k+1} = H_k h_k
             }
 #pragma unroll
             for (int c4 = 0; c4 < NUP; c4 += 4) {
@@ -223,16 +238,18 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
                     for (int q = 0; q < 4; ++q) if (NX + c4 + q < NBP) du[r] += U[r][NX + c4 + q] * r4[q];   // Delta u_k = M_k rhs (u-rows)
             }
+            T xs[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                own[OX + r] = x[r];
-                if (isu[r]) own[ODU - NX + r] = du[r];
+                xs[r] = x[r][0] + x[r][1];
+                own[OX + r] = xs[r];
+                if (!isx[r]) own[ODU - NX + r] = du[r];
             }
             __syncthreads();
             // steps 2-4
-            T dot[R], avx[R];
+            T dot[R][2], avx[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { dot[r] = (T)0; avx[r] = (T)0; }
+            for (int r = 0; r < R; ++r) { dot[r][0] = dot[r][1] = (T)0; avx[r] = (T)0; }
 #pragma unroll
             for (int c4 = 0; c4 < NBP; c4 += 4) {
                 T x4[4];
@@ -240,7 +257,7 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) dot[r] += U[r][c4 + q] * x4[q];           // [A_k B_k] xbar_k (x-rows)
+                    for (int q = 0; q < 4; ++q) dot[r][q & 1] += U[r][c4 + q] * x4[q];    // [A_k B_k] xbar_k (x-rows)
             }
 #pragma unroll
             for (int c4 = 0; c4 < NUP; c4 += 4) {
@@ -255,22 +272,26 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const T xpi = own[-SS + OX + r];
+                const T duu = isx[r] ? (T)0 : du[r];
                 const T av = (isx[r] ? avx[r] : du[r]) + beh[r];                 // a = Bbar du + betahat
-                const T bv = (isx[r] ? dot[r] + ev[r] : xpi) - lah[r];           // b = Abar xbar_k + ebar - lambdahat
+                const T bv = (isx[r] ? dot[r][0] + dot[r][1] + ev[r] : xpi) - lah[r];   // b = Abar xbar_k + ebar - lambdahat
                 const T gam = av - bv;
-                const T zn = clipv(((T)2 * (x[r] + thh[r] + bv) + gam) * (T)(1.0 / 3.0), lo[r], hi[r]);
+                const T zn = clipv(((T)2 * (xs[r] + thh[r] + bv) + gam) * (T)(1.0 / 3.0), lo[r], hi[r]);
                 const T vn = (T)0.5 * (zn + gam);
-                const T thn = thh[r] + x[r] - zn;
+                const T thn = thh[r] + xs[r] - zn;
                 const T ben = av - vn;
                 const T lan = zn - bv - vn;
                 const T d0 = thn - thh[r], d1 = ben - beh[r], d2 = lan - lah[r], d3 = zn - zh[r], d4 = vn - vh[r];
                 const T d5 = (zn - vn) - (zh[r] - vh[r]);
-                T a = d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
-                const T dn = clipv(du[r] + deh[r], dlo[r], dhi[r]);             // Delta-u box copy (reading R12), u-rows
-                const T den = deh[r] + du[r] - dn;
-                const T e0 = den - deh[r], e1 = dn - dh[r];
-                if (has_du && isu[r]) { a += e0 * e0 + e1 * e1; prv.d[r] = dn; prv.de[r] = den; }
-                if (isx[r] || isu[r]) { acc += a; prv.z[r] = zn; prv.v[r] = vn; prv.th[r] = thn; prv.be[r] = ben; prv.la[r] = lan; }
+                acc += d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
+                prv.z[r] = zn; prv.v[r] = vn; prv.th[r] = thn; prv.be[r] = ben; prv.la[r] = lan;
+                if (DU) {                                                      // Delta-u box copy (reading R12); x-rows: zeros
+                    const T dn = clipv(duu + deh[r], own[OC + 2 * C::ROWP + r], own[OC + 3 * C::ROWP + r]);
+                    const T den = deh[r] + duu - dn;
+                    const T e0 = den - deh[r], e1 = dn - dh[r];
+                    acc += e0 * e0 + e1 * e1;
+                    prv.d[r] = dn; prv.de[r] = den;
+                }
             }
             // step 4: c = rho * sum (fixed order: group butterfly in T, then double)
 #pragma unroll
@@ -281,36 +302,36 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             if (lane == 0) red[warp] = s;
             __syncthreads();
             s = lane < nwarps ? red[lane] : 0.0;
+            const double c_prev = red[32 + (par ^ 1)];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
             // steps 5-7; every thread decides from the same bits
             const double c = p.rho * s;
-            if (tid == 0) red[33] = c;
             it_done = it + 1;
             const bool stop = p.tol > 0.0 && c < p.tol;
             const bool accept = !stop && c <= p.eta * c_prev;
-            if (tid == 0 && p.hist_c && it < p.hist_cap) {
-                p.hist_c[(size_t)b * p.hist_cap + it] = c;
-                p.hist_a[(size_t)b * p.hist_cap + it] = (unsigned char)accept;
+            if (tid == 0) {
+                red[32 + par] = c;
+                if (!accept && !stop) ++sCnt[0];
+                if (hc && it < p.hist_cap) { hc[it] = c; ha[it] = (unsigned char)accept; }
             }
             if (stop) { done = true; return true; }
             if (accept) {
                 kap = jacc < C::KAPN ? sKap[jacc] : (T)kappa_tab[jacc];
                 ++jacc;
             } else {
-                kap = (T)0; jacc = 0; ++restarts;
+                kap = (T)0; jacc = 0;
             }
-            c_prev = c;
             return false;
         };
 
         __syncthreads();
         bool in_b = false;                       // which of (sa, sb) holds the current iterate
         for (int it = 0; it < iters; it += 2) {
-            if (iteration(sa, sb, it)) { in_b = true; break; }
+            if (iteration(sa, sb, it, 0)) { in_b = true; break; }
             in_b = true;
             if (it + 1 >= iters) break;
-            if (iteration(sb, sa, it + 1)) { in_b = false; break; }
+            if (iteration(sb, sa, it + 1, 1)) { in_b = false; break; }
             in_b = false;
         }
         if (in_b) sa = sb;                       // register moves; a reference select would force local memory
@@ -320,21 +341,25 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int i = li * R + r;
-            if (isx[r] || isu[r]) {
-                T *rec = p.S + (size_t)ctl0.i_cur * p.buf_stride + p.st(b, k);
+            if (stage_ok && i < NB) {
+                T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(b, k);
                 rec[p.oZ() + i] = fin.z[r]; rec[p.oV() + i] = fin.v[r]; rec[p.oTH() + i] = fin.th[r];
                 rec[p.oBE() + i] = fin.be[r]; rec[p.oLA() + i] = fin.la[r];
                 p.X[sk * NB + i] = own[OX + r];
-                if (isu[r]) {
+                if (i >= NX) {
                     p.DU[sk * NU + (i - NX)] = own[ODU - NX + r];
-                    if (has_du) { rec[p.oD() + (i - NX)] = fin.d[r]; rec[p.oDE() + (i - NX)] = fin.de[r]; }
+                    if (DU) { rec[p.oD() + (i - NX)] = fin.d[r]; rec[p.oDE() + (i - NX)] = fin.de[r]; }
                 }
             }
         }
+        __syncthreads();                         // red[], sCnt of the last iteration are visible to thread 0
         if (tid == 0) {
-            InstCtl c = ctl0;
-            c.alpha = alpha_tab[jacc]; c.c_prev = c_prev; c.c_last = red[33]; c.kappa = (double)kap;
-            c.done = done ? 1 : 0; c.iters = it_done; c.restarts = restarts;
+            InstCtl c = p.ctl[b];
+            const int last = (it_done - 1) & 1;
+            c.alpha = alpha_tab[jacc]; c.c_last = it_done ? red[32 + last] : p.c0;
+            c.c_prev = done ? red[32 + (last ^ 1)] : c.c_last;
+            c.kappa = (double)kap;
+            c.done = done ? 1 : 0; c.iters = it_done; c.restarts = sCnt[0];
             p.ctl[b] = c;
         }
         __syncthreads();
@@ -345,7 +370,7 @@ template <typename T, int NX, int NU, int R, int MAXT>
 int launch_resident(pimpc_s *h, int iters, double tol, int nwarps)
 {
     using C = RCfg<T, NX, NU, R>;
-    auto kern = k_resident<T, NX, NU, R, MAXT>;
+    auto kern = h->has_du ? k_resident<T, NX, NU, R, MAXT, true> : k_resident<T, NX, NU, R, MAXT, false>;
     const size_t smem = C::smem_bytes(nwarps);
     PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;

@@ -188,7 +188,7 @@ Prob<T> make_prob(pimpc_s *h, double tol)
 {
     Prob<T> p{};
     p.nx = h->nx; p.nu = h->nu; p.nb = h->nb; p.N = h->N; p.batch = h->batch; p.rec = h->rec;
-    p.has_du = h->has_du; p.has_e = h->has_e;
+    p.has_du = h->has_du; p.has_e = h->has_e; p.has_q = h->has_q;
     p.A = (const T *)h->A; p.B = (const T *)h->B; p.e = h->has_e ? (const T *)h->e : nullptr;
     p.x0 = (const T *)h->x0; p.uprev = (const T *)h->uprev;
     p.Q = (const T *)h->Q; p.R = (const T *)h->R;

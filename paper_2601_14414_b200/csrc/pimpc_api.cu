@@ -313,7 +313,7 @@ int pimpc_set_cost(pimpc_t h, const void *Q, const void *R, const void *P, const
     if (Wdu) { rc = copy_in(h, h->Wdu, Wdu, rep * nr * esz); if (rc) return rc; }
     if (qbar) { rc = copy_in(h, h->qbar, qbar, rep * h->nb * esz); if (rc) return rc; }
     else PIMPC_CUDA_TRY(h, cudaMemsetAsync(h->qbar, 0, (size_t)h->batch * h->nb * esz, h->stream));
-    h->has_P = P != nullptr; h->has_wdu = Wdu != nullptr;
+    h->has_P = P != nullptr; h->has_wdu = Wdu != nullptr; h->has_q = qbar != nullptr;
     h->cost_per_instance = per_instance ? 1 : 0;
     h->cache_dirty = true;
     return PIMPC_OK;

@@ -27,7 +27,7 @@ enum { PIMPC_DEVERR_NONFINITE = 1, PIMPC_DEVERR_NOTPD = 2 };
 template <typename T>
 struct Prob {
     int nx, nu, nb, N, batch, rec;
-    int has_du, has_e;
+    int has_du, has_e, has_q;        // has_q: a linear cost term qbar was supplied
     const T *A, *B, *e;              // [batch][N][nx][nx], [batch][N][nx][nu], [batch][N][nx] or null
     const T *x0, *uprev;             // [batch][nx], [batch][nu]
     const T *Q, *R, *P, *Wdu, *qbar; // cost; P, Wdu may be null; stride 0 = shared by all instances
@@ -74,7 +74,7 @@ struct pimpc_s {
     int cost_per_instance = 0;
     void *lo = nullptr, *hi = nullptr, *dlo = nullptr, *dhi = nullptr;
     int bnd_per_instance = 0;
-    int has_du = 0, has_e = 0, has_P = 0, has_wdu = 0;
+    int has_du = 0, has_e = 0, has_P = 0, has_wdu = 0, has_q = 0;
     void *H = nullptr, *M = nullptr, *S = nullptr, *X = nullptr, *DU = nullptr;
     InstCtl *ctl = nullptr;
     double *partial = nullptr;
