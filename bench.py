@@ -56,6 +56,18 @@ def peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
+def ncu_traffic(engine, config):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture (profiles/traffic.csv)."""
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tp):
+        return None
+    for line in open(tp).read().splitlines()[1:]:
+        f = line.split(",")
+        if len(f) >= 4 and f[0] == str(engine) and f[1] == config:
+            return int(f[3])
+    return None
+
+
 def alu_peak_tflops(dtype, sm_mhz, sms=148):
     lanes = 128 if dtype == "f32" else 64          # FP32 / FP64 FMA lanes per SM (DESIGN.md)
     return sms * lanes * 2 * sm_mhz * 1e6 / 1e12
@@ -307,9 +319,7 @@ def main():
         (" hbm_gbs" if roof["bound"] == "hbm" else " sm_max_mhz x 148 SM x 128 FP32 lanes x 2 (DESIGN.md)")
     roof["kernel_ms_per_launch"] = k_ms
     roof["cache_kernel_ms"] = statistics.mean(setup_ms)
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        roof["traffic"] = json.load(open(tp)).get(str(engine))
+    roof["traffic"] = ncu_traffic(engine, "C4_f32")
 
     h2d = A_h.numel() * 4 + B_h.numel() * 4 + x0_h.numel() * 4
     d2h = (x_h.numel() + u_h.numel() + du_h.numel()) * 4 + res_h.numel()
