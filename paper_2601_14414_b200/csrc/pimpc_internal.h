@@ -89,7 +89,9 @@ struct pimpc_s {
     int tab_cap = 0;
     // engine-private storage (packed blobs of the STREAM engine etc.)
     void *blob = nullptr;
-    size_t blob_stride = 0;
+    size_t blob_bytes = 0;
+    double *spartial = nullptr;              // [2][grid][MAXI] partial sums of c of the STREAM engine
+    size_t spartial_cap = 0;
     bool blob_dirty = true;
 
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // before cache kernel, before iteration, after iteration
@@ -110,6 +112,8 @@ int launch_begin(pimpc_s *h);                       // Alg. 1 input: alpha=1, c_
 int run_staged(pimpc_s *h, int iters, double tol);  // v0 engine
 int run_resident(pimpc_s *h, int iters, double tol);
 bool resident_supported(const pimpc_s *h, std::string *why);
+int run_stream(pimpc_s *h, int iters, double tol);
+bool stream_supported(const pimpc_s *h, std::string *why);
 int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res_dev);
 int launch_state_io(pimpc_s *h, int which, void *buf_dev, int set);
 int launch_zero_state(pimpc_s *h);

@@ -115,6 +115,60 @@ def test_config5_full_size_sampled(oracle, pimpc, dtype):
         parity.check_instance(oracle, p, dtype, g, b)
 
 
+# ---- STREAM engine (persistent cooperative grid, bulk-copy ring): ranges that split instances ------
+@pytest.fixture
+def stream_grid(monkeypatch):
+    def set_(n):
+        if n:
+            monkeypatch.setenv("PIMPC_STREAM_GRID", str(n))
+        else:
+            monkeypatch.delenv("PIMPC_STREAM_GRID", raising=False)
+    return set_
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("grid", [0, 1, 3, 7])
+@pytest.mark.parametrize("shape", [(48, 12, 37, 3), (12, 4, 41, 2), (4, 2, 23, 5)])
+def test_stream_engine_all_options(oracle, pimpc, stream_grid, shape, grid, dtype):
+    """grid = 0: one or two steps per CTA (every step a halo); 1: one CTA owns everything; 3, 7: ranges
+    start inside instances and span several of them."""
+    nx, nu, N, batch = shape
+    stream_grid(grid)
+    p = wl.random_ltv(nx, nu, N, batch, seed=nx * 10 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
+                      qbar=True, bounds=0.8, du_bound=0.5)
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="stream", iters=120, tol=0.0)
+    assert g["info"]["engine"] == pimpc.ENGINE_STREAM
+    parity.check_properties(p, dtype, g)
+
+
+@pytest.mark.parametrize("grid", [0, 5])
+def test_stream_engine_unbounded_and_plain_admm(oracle, pimpc, stream_grid, grid):
+    stream_grid(grid)
+    p = wl.random_ltv(4, 2, 9, 2, seed=77, affine=True, bounds=None, du_bound=None)
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="stream", iters=300, tol=0.0)
+    assert "D" not in g
+    p = wl.quadrotor_ltv(12, 2, iters=120, tol=0.0)
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="stream", eta=0.0)
+    assert np.all(g["res"]["restarts"] == 120)
+
+
+@pytest.mark.parametrize("grid", [0, 4])
+def test_stream_engine_early_stop_and_warm_start(oracle, pimpc, stream_grid, grid):
+    stream_grid(grid)
+    p = wl.quadrotor_ltv(8, 6, iters=3000, tol=1e-4, rho=10.0, name="tolbatch")
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="stream")
+    assert len(set(g["res"]["iters"].tolist())) > 1 and np.all(g["res"]["converged"] == 1)
+    p = wl.quadrotor_ltv(9, 2, iters=40, tol=0.0)
+    s = pimpc.Solver(p.nx, p.nu, p.N, p.batch, dtype="f64", engine="stream")
+    s.set_problem(p); s.solve(40)
+    warm = {k: s.get_state(k) for k in ("Z", "V", "TH", "BE", "LA", "D", "DE")}
+    s.solve(25)
+    z2 = s.get_state("Z")
+    for b in range(p.batch):
+        o = parity.oracle_run(oracle, p, "f64", b, iters=25, tol=0.0, warm=warm)
+        assert parity.relerr(z2[b], o.Z) <= 1e-9
+
+
 # ---- odd shapes, optional terms, edge cases -----------------------------------------------------
 @pytest.mark.parametrize("engine", ENGINES_SMALL)
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
