@@ -1,0 +1,541 @@
+// COOP engine: Algorithm 1 for ONE long-horizon instance (batch = 1; C2, C3) with
+// the whole problem resident on chip, spread over the SMs, and ONE cooperative launch per solve.
+//   * CTA c owns the contiguous stages [k0, k1) of the horizon.  Their matrices (H_k, [A_k B_k], M_k)
+//     are read from HBM once per solve into shared memory; their iterates (current and previous) live in
+//     registers; a group of LPS lanes owns a stage (lane = row), SPG stages per group.
+//   * The neighbour coupling across a CTA boundary costs no extra barrier: the stage before the range
+//     is a "ghost" whose xbar_{k0} = H_{k0-1} h_{k0-1} is recomputed here (its H is resident too), and the
+//     stage after the range is a ghost that only supplies w_{k1}.  The ghosts' iterates (z, theta) /
+//     (z, v, lambda) arrive from the neighbour CTA as tagged words in global memory.
+//   * The ONLY global exchange per iteration is data-flow, not a barrier: every CTA publishes its partial
+//     sum of c (step 4) and its boundary iterates as {value, iteration tag} words
+//     (8-byte single-copy-atomic stores, no fences); a communication warp polls the partials of all
+//     CTAs, sums them in a fixed order (bit-identical in every CTA) and every thread takes the same
+//     accept / restart decision (steps 5-7).  Buffers are double-buffered on the
+//     iteration parity: a CTA cannot run two iterations ahead of a neighbour because it needs that
+//     neighbour's next partial first.
+// The launch is cooperative only to guarantee co-residency of the polling CTAs.
+#include <algorithm>
+#include <cstdlib>
+
+#include "pimpc_internal.h"
+
+namespace {
+
+__host__ __device__ constexpr int pow2ceil_o(int v) { int p = 1; while (p < v) p <<= 1; return p; }
+__host__ __device__ constexpr int round4_o(int v) { return (v + 3) / 4 * 4; }
+
+// ---- tagged words: {value bits, tag}; 8-byte parts are single-copy atomic, each part carries its own tag ----
+template <typename T> struct Tagged;
+template <> struct Tagged<float> {
+    typedef uint2 W;
+    static __device__ __forceinline__ void st(W *p, float v, uint32_t tag)
+    {
+        asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(__float_as_uint(v)), "r"(tag) : "memory");
+    }
+    static __device__ __forceinline__ bool ld(const W *p, uint32_t tag, float &v)
+    {
+        uint32_t a, b;
+        asm volatile("ld.relaxed.gpu.global.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "l"(p) : "memory");
+        v = __uint_as_float(a);
+        return b == tag;
+    }
+};
+template <> struct Tagged<double> {
+    typedef uint4 W;
+    static __device__ __forceinline__ void st(W *p, double v, uint32_t tag)
+    {
+        const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
+        asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag) : "memory");
+    }
+    static __device__ __forceinline__ bool ld(const W *p, uint32_t tag, double &v)
+    {
+        uint32_t a, b, c, d;
+        asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(p) : "memory");
+        v = __hiloint2double((int)c, (int)a);
+        return b == tag && d == tag;
+    }
+};
+
+__device__ __forceinline__ void ld4o(const float *p, float (&o)[4])
+{
+    const float4 v = *reinterpret_cast<const float4 *>(p);
+    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void ld4o(const double *p, double (&o)[4])
+{
+    const double2 a = *reinterpret_cast<const double2 *>(p), b = *reinterpret_cast<const double2 *>(p + 2);
+    o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
+}
+template <typename T> __device__ __forceinline__ T clipo(T v, T lo, T hi) { return fmin(fmax(v, lo), hi); }
+
+template <typename T, int NX, int NU>
+struct OCfg {
+    static constexpr int NB = NX + NU;
+    static constexpr int LPS = pow2ceil_o(NB);                 // lanes per stage (one row per lane)
+    static constexpr int NBP = round4_o(NB), NUP = round4_o(NU);
+    static constexpr int WPE = sizeof(T) / 4;                  // 32-bit words per element
+    static constexpr int HS = NBP + 4 / WPE;                   // matrix row stride: 16-byte row reads of consecutive lanes hit disjoint banks
+    static constexpr int KAPN = 1024;
+    static constexpr int MAXJ = 5;                             // partials polled per lane of the communication warp: grid <= 160
+    // one block per virtual slot v = 0..L+1 (stage k0 - 1 + v):
+    //   W w_k = zhat - vhat - ebar + lambdahat   X xbar_{k+1}   D vhat - betahat   HH h_k   RH rhs of the Delta-u update
+    //   DU Delta u_k   E e_k   HM H_k [NB][HS]   AB [A_k B_k] [NX][HS]   MM M_k [NU][NUP]
+    static constexpr int OW = 0, OX = LPS, OD = 2 * LPS, OHH = 3 * LPS, ORH = 4 * LPS, ODU = ORH + NUP, OE = ODU + NUP,
+                         OHM = OE + LPS, OAB = OHM + NB * HS, OMM = OAB + NX * HS, SS0 = OMM + NU * NUP;
+    // slot stride == LPS words (mod 32): the groups of a warp work on consecutive slots and hit disjoint banks
+    static constexpr int SSW0 = SS0 * WPE;
+    static constexpr int SSW = SSW0 + ((LPS - SSW0 % 32) + 32) % 32;
+    static constexpr int SS = SSW / WPE;
+    static_assert(SSW % WPE == 0 && SS % 4 == 0 && LPS <= 32 && NX % 4 == 0, "slot layout");
+    static constexpr size_t head_bytes = 40 * sizeof(double) + (KAPN + 2 * LPS + 2 * NUP) * sizeof(T);
+    static size_t smem_bytes(int slots) { return head_bytes + (size_t)slots * SS * sizeof(T); }
+    // exchange buffers per CTA and parity (tagged words): to the left neighbour (z, v, lambda) of the first stage,
+    // to the right neighbour (z, theta) of the last stage
+    static constexpr int HALO = 5 * LPS;
+};
+
+template <typename T> struct OState { T z, v, th, be, la, d, de; };
+
+template <typename T, int NX, int NU, int SPG, int MAXT, bool DU>
+__global__ void __launch_bounds__(MAXT, 1)
+k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__restrict__ kappa_tab, const int iters,
+       typename Tagged<double>::W *__restrict__ part, typename Tagged<T>::W *__restrict__ halo)
+{
+    using C = OCfg<T, NX, NU>;
+    using TW = Tagged<T>;
+    using TD = Tagged<double>;
+    constexpr int NB = C::NB, LPS = C::LPS, NBP = C::NBP, NUP = C::NUP, HS = C::HS, SS = C::SS;
+    constexpr int OW = C::OW, OX = C::OX, OD = C::OD, OHH = C::OHH, ORH = C::ORH, ODU = C::ODU, OE = C::OE, OHM = C::OHM,
+                  OAB = C::OAB, OMM = C::OMM;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *red = reinterpret_cast<double *>(smem_raw);        // [32] warp partials, [32..33] c of the last two iterations
+    T *sKap = reinterpret_cast<T *>(red + 40);                 // [KAPN]
+    T *sQ = sKap + C::KAPN;                                    // [LPS] qbar
+    T *sDlo = sQ + LPS, *sDhi = sDlo + NUP;                    // [NUP] Delta-u box
+    T *sBlk = sDhi + NUP + (LPS - 2 * NUP % LPS) % LPS;        // [L+2][SS]   (head_bytes reserves 2 LPS + 2 NUP)
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int ncw = nwarps - 1;                                // compute warps; the last warp is the communication warp
+    const bool comm = warp == ncw;
+    const int ngroups = ncw * (32 / LPS);
+    const int g = tid / LPS, li = tid % LPS;
+    const int N = p.N, G = gridDim.x, cta = blockIdx.x;
+    const int k0 = (int)((long long)cta * N / G), k1 = (int)((long long)(cta + 1) * N / G), L = k1 - k0;
+    const bool has_left = k0 > 0, has_right = k1 < N;
+    const T rho = (T)p.rho;
+    const bool has_e = p.e != nullptr, has_q = p.has_q != 0;
+    const bool rowok = li < NB, isx = li < NX || !rowok;       // pad lanes take the x-row path with zeros
+    const int i_cur = p.ctl[0].i_cur;
+
+    // ---- once per solve: stage matrices -> shared memory, iterates -> registers ----------------------------
+    for (int i = tid; i < (L + 2) * SS; i += blockDim.x) sBlk[i] = (T)0;
+    for (int i = tid; i < min(iters + 1, C::KAPN); i += blockDim.x) sKap[i] = (T)kappa_tab[i];
+    if (tid < LPS) sQ[tid] = tid < NB ? p.qbar[tid] : (T)0;
+    if (tid < NUP) {
+        sDlo[tid] = (DU && tid < NU) ? p.dlo[tid] : (T)0;
+        sDhi[tid] = (DU && tid < NU) ? p.dhi[tid] : (T)0;
+    }
+    if (tid == 0) { red[32] = p.c0; red[33] = p.c0; }
+    __syncthreads();
+    for (int v = 0; v <= L + 1; ++v) {
+        const int k = k0 - 1 + v;
+        if (k < 0 || k >= N) continue;
+        T *blk = sBlk + (size_t)v * SS;
+        if (v <= L)                                            // H_k: real stages and the left ghost
+            for (int i = tid; i < NB * NB; i += blockDim.x) blk[OHM + (i / NB) * HS + i % NB] = p.H[(size_t)k * NB * NB + i];
+        if (v >= 1) {                                          // [A_k B_k], e_k: real stages and the right ghost
+            for (int i = tid; i < NX * NX; i += blockDim.x) blk[OAB + (i / NX) * HS + i % NX] = p.A[(size_t)k * NX * NX + i];
+            for (int i = tid; i < NX * NU; i += blockDim.x) blk[OAB + (i / NU) * HS + NX + i % NU] = p.B[(size_t)k * NX * NU + i];
+            if (has_e && tid < NX) blk[OE + tid] = p.e[(size_t)k * NX + tid];
+        }
+        if (v >= 1 && v <= L)
+            for (int i = tid; i < NU * NU; i += blockDim.x) blk[OMM + (i / NU) * NUP + i % NU] = p.M[(size_t)k * NU * NU + i];
+    }
+    if (!has_left && tid < LPS)                                // slot 0 of the first CTA: xbar_0 = (x(t); u(t-1))
+        sBlk[OX + tid] = tid < NX ? p.x0[tid] : (tid < NB ? p.uprev[tid - NX] : (T)0);
+
+    OState<T> sa[SPG], sb[SPG];
+    T lo[SPG], hi[SPG];
+    bool exist[SPG], real[SPG], ghl[SPG], ghr[SPG];
+    T *blkp[SPG];
+#pragma unroll
+    for (int s = 0; s < SPG; ++s) {
+        const int v = s * ngroups + g, k = k0 - 1 + v;
+        exist[s] = !comm && v <= L + 1;
+        real[s] = exist[s] && v >= 1 && v <= L;
+        ghl[s] = exist[s] && v == 0 && has_left;
+        ghr[s] = exist[s] && v == L + 1 && has_right;
+        blkp[s] = sBlk + (size_t)(exist[s] ? v : 0) * SS;
+        const bool ok = (real[s] || ghl[s] || ghr[s]) && rowok;
+        const T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(0, ok ? k : 0);
+        const bool oku = ok && li >= NX;
+        sa[s].z = ok ? rec[p.oZ() + li] : (T)0;
+        sa[s].v = ok ? rec[p.oV() + li] : (T)0;
+        sa[s].th = ok ? rec[p.oTH() + li] : (T)0;
+        sa[s].be = ok ? rec[p.oBE() + li] : (T)0;
+        sa[s].la = ok ? rec[p.oLA() + li] : (T)0;
+        sa[s].d = (oku && DU) ? rec[p.oD() + (li - NX)] : (T)0;
+        sa[s].de = (oku && DU) ? rec[p.oDE() + (li - NX)] : (T)0;
+        sb[s] = sa[s];
+        lo[s] = (real[s] && rowok) ? p.lo[li] : (T)0;
+        hi[s] = (real[s] && rowok) ? p.hi[li] : (T)0;
+    }
+    const int hrow = rowok ? li : NB - 1;                      // clamped row indices of pad / u lanes (results unused)
+    const int xrow = li < NX ? li : NX - 1;
+    const int mrow = (li >= NX && rowok) ? li - NX : 0;
+    const bool ulane = li >= NX && rowok;
+
+    T kap = (T)0;
+    int jacc = 0, it_done = 0, restarts = 0;
+    bool done = false;
+    __syncthreads();
+
+    // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.  par = it & 1.
+    auto iteration = [&](OState<T> (&cur)[SPG], OState<T> (&prv)[SPG], const int it, const int par) -> bool {
+        const uint32_t tag = (uint32_t)it + 1u;
+        T zh[SPG], vh[SPG], thh[SPG], beh[SPG], lah[SPG], dh[SPG], deh[SPG], dv[SPG], ev[SPG];
+        // ---- A: steps 6/7 of the previous iteration: hats from (cur, prev, kappa); w, vhat - betahat ----
+#pragma unroll
+        for (int s = 0; s < SPG; ++s) {
+            zh[s] = cur[s].z + kap * (cur[s].z - prv[s].z);
+            vh[s] = cur[s].v + kap * (cur[s].v - prv[s].v);
+            thh[s] = cur[s].th + kap * (cur[s].th - prv[s].th);
+            beh[s] = cur[s].be + kap * (cur[s].be - prv[s].be);
+            lah[s] = cur[s].la + kap * (cur[s].la - prv[s].la);
+            if (DU) {
+                dh[s] = cur[s].d + kap * (cur[s].d - prv[s].d);
+                deh[s] = cur[s].de + kap * (cur[s].de - prv[s].de);
+            }
+            dv[s] = vh[s] - beh[s];
+            T w = zh[s] - vh[s] + lah[s];
+            ev[s] = (T)0;
+            if (has_e && exist[s]) { ev[s] = blkp[s][OE + li]; w -= ev[s]; }
+            if (exist[s]) { blkp[s][OW + li] = w; blkp[s][OD + li] = dv[s]; }
+        }
+        __syncthreads();
+        // ---- B: step 1: g = Abar_{k+1}^T w_{k+1}, h_k; rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat] ----
+#pragma unroll
+        for (int s = 0; s < SPG; ++s) {
+            if (!(real[s] || ghl[s])) continue;
+            const T *blk = blkp[s], *nxt = blk + SS;
+            T g0 = (T)0, g1 = (T)0, r0 = (T)0, r1 = (T)0;
+#pragma unroll
+            for (int c4 = 0; c4 < NX; c4 += 4) {
+                T w4[4], d4[4];
+                ld4o(nxt + OW + c4, w4);
+                ld4o(blk + OD + c4, d4);
+#pragma unroll
+                for (int q = 0; q < 4; q += 2) {
+                    g0 += nxt[OAB + (c4 + q) * HS + li] * w4[q];
+                    g1 += nxt[OAB + (c4 + q + 1) * HS + li] * w4[q + 1];
+                    r0 += blk[OAB + (c4 + q) * HS + li] * d4[q];
+                    r1 += blk[OAB + (c4 + q + 1) * HS + li] * d4[q + 1];
+                }
+            }
+            T gg = g0 + g1;
+            if (!isx) gg += nxt[OW + li];                                    // the [0 I] rows of Abar_{k+1}
+            T hh = rho * (zh[s] - thh[s]) + rho * gg;                        // h_k (index reading R2)
+            if (has_q) hh += sQ[li];
+            blkp[s][OHH + li] = hh;
+            T rr = r0 + r1 + dv[s];
+            if (DU) rr += dh[s] - deh[s];
+            if (ulane) blkp[s][ORH + li - NX] = rr;
+        }
+        __syncwarp();
+        // ---- C: xbar_{k+1} = H_k h_k; Delta u_k = M_k rhs ----
+        T xs[SPG], du[SPG];
+#pragma unroll
+        for (int s = 0; s < SPG; ++s) {
+            xs[s] = (T)0; du[s] = (T)0;
+            if (!(real[s] || ghl[s])) continue;
+            const T *blk = blkp[s];
+            T x0 = (T)0, x1 = (T)0;
+#pragma unroll
+            for (int c4 = 0; c4 < NBP; c4 += 4) {
+                T h4[4], m4[4];
+                ld4o(blk + OHH + c4, h4);
+                ld4o(blk + OHM + hrow * HS + c4, m4);
+                x0 += m4[0] * h4[0]; x1 += m4[1] * h4[1]; x0 += m4[2] * h4[2]; x1 += m4[3] * h4[3];
+            }
+            xs[s] = rowok ? x0 + x1 : (T)0;
+            blkp[s][OX + li] = xs[s];
+            if (real[s]) {
+                T d0 = (T)0;
+#pragma unroll
+                for (int c4 = 0; c4 < NUP; c4 += 4) {
+                    T r4[4], m4[4];
+                    ld4o(blk + ORH + c4, r4);
+                    ld4o(blk + OMM + mrow * NUP + c4, m4);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) d0 += m4[q] * r4[q];
+                }
+                du[s] = ulane ? d0 : (T)0;
+                if (ulane) blkp[s][ODU + li - NX] = du[s];
+            }
+        }
+        __syncthreads();
+        // ---- D: steps 2-4 of the real stages ----
+        T acc = (T)0;
+#pragma unroll
+        for (int s = 0; s < SPG; ++s) {
+            if (!real[s]) continue;
+            const T *blk = blkp[s], *prvb = blk - SS;
+            T t0 = (T)0, t1 = (T)0, avx = (T)0;
+#pragma unroll
+            for (int c4 = 0; c4 < NBP; c4 += 4) {
+                T x4[4], a4[4];
+                ld4o(prvb + OX + c4, x4);
+                ld4o(blk + OAB + xrow * HS + c4, a4);
+                t0 += a4[0] * x4[0]; t1 += a4[1] * x4[1]; t0 += a4[2] * x4[2]; t1 += a4[3] * x4[3];   // [A_k B_k] xbar_k (x-rows)
+                if (c4 >= NX) {
+                    T u4[4];
+                    ld4o(blk + ODU + (c4 - NX), u4);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) avx += a4[q] * u4[q];                                  // B_k Delta u_k (x-rows)
+                }
+            }
+            const bool xr = li < NX;
+            const T xpi = prvb[OX + li];
+            const T duu = isx ? (T)0 : du[s];
+            const T av = (isx ? (xr ? avx : (T)0) : du[s]) + beh[s];                    // a = Bbar du + betahat
+            const T bv = (isx ? (xr ? t0 + t1 + ev[s] : (T)0) : xpi) - lah[s];          // b = Abar xbar_k + ebar - lambdahat
+            const T gam = av - bv;
+            const T zn = clipo(((T)2 * (xs[s] + thh[s] + bv) + gam) * (T)(1.0 / 3.0), lo[s], hi[s]);   // Thm 1 (proof form, R1)
+            const T vn = (T)0.5 * (zn + gam);
+            const T thn = thh[s] + xs[s] - zn;
+            const T ben = av - vn;
+            const T lan = zn - bv - vn;
+            const T d0 = thn - thh[s], d1 = ben - beh[s], d2 = lan - lah[s], d3 = zn - zh[s], d4 = vn - vh[s];
+            const T d5 = (zn - vn) - (zh[s] - vh[s]);
+            acc += d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
+            prv[s].z = zn; prv[s].v = vn; prv[s].th = thn; prv[s].be = ben; prv[s].la = lan;
+            if (DU) {                                                          // Delta-u box copy (reading R12); x-rows: zeros
+                const T dn = clipo(duu + deh[s], isx ? (T)0 : sDlo[mrow], isx ? (T)0 : sDhi[mrow]);
+                const T den = deh[s] + duu - dn;
+                const T e0 = den - deh[s], e1 = dn - dh[s];
+                acc += e0 * e0 + e1 * e1;
+                prv[s].d = dn; prv[s].de = den;
+            }
+            // boundary iterates for the neighbour CTAs' ghosts (tagged words, parity-double-buffered)
+            const int v = s * ngroups + g;
+            if (v == 1 && has_left) {
+                typename TW::W *o = halo + ((size_t)par * G + cta) * C::HALO;
+                TW::st(o + li, zn, tag); TW::st(o + LPS + li, vn, tag); TW::st(o + 2 * LPS + li, lan, tag);
+            }
+            if (v == L && has_right) {
+                typename TW::W *o = halo + ((size_t)par * G + cta) * C::HALO + 3 * LPS;
+                TW::st(o + li, zn, tag); TW::st(o + LPS + li, thn, tag);
+            }
+        }
+        // ---- step 4: c = rho * sum (fixed order: group butterfly in T, then double) ----
+#pragma unroll
+        for (int o = LPS / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        double sum = (double)acc;
+#pragma unroll
+        for (int o = 16; o >= LPS; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if (lane == 0 && !comm) red[warp] = sum;
+        __syncthreads();
+        if (comm) {
+            sum = lane < ncw ? red[lane] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            typename TD::W *pp = part + (size_t)par * G;
+            if (lane == 0) TD::st(pp + cta, sum, tag);
+            double vals[C::MAXJ];
+            bool got[C::MAXJ];
+#pragma unroll
+            for (int u = 0; u < C::MAXJ; ++u) { vals[u] = 0.0; got[u] = lane + 32 * u >= G; }
+            bool all;
+            do {
+                all = true;
+#pragma unroll
+                for (int u = 0; u < C::MAXJ; ++u) {
+                    if (!got[u]) { got[u] = TD::ld(pp + lane + 32 * u, tag, vals[u]); all = all && got[u]; }
+                }
+            } while (!all);
+            sum = 0.0;
+#pragma unroll
+            for (int u = 0; u < C::MAXJ; ++u) sum += vals[u];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            if (lane == 0) red[32 + par] = p.rho * sum;
+        } else {
+            // the ghosts' new iterates, published by the neighbours in their phase D of this iteration
+#pragma unroll
+            for (int s = 0; s < SPG; ++s) {
+                if (ghl[s] && rowok) {
+                    const typename TW::W *o = halo + ((size_t)par * G + cta - 1) * C::HALO + 3 * LPS;
+                    T a, b2;
+                    bool ga = false, gb = false;
+                    do { if (!ga) ga = TW::ld(o + li, tag, a); if (!gb) gb = TW::ld(o + LPS + li, tag, b2); } while (!(ga && gb));
+                    prv[s].z = a; prv[s].th = b2;
+                }
+                if (ghr[s] && rowok) {
+                    const typename TW::W *o = halo + ((size_t)par * G + cta + 1) * C::HALO;
+                    T a, b2, c2;
+                    bool ga = false, gb = false, gc = false;
+                    do {
+                        if (!ga) ga = TW::ld(o + li, tag, a);
+                        if (!gb) gb = TW::ld(o + LPS + li, tag, b2);
+                        if (!gc) gc = TW::ld(o + 2 * LPS + li, tag, c2);
+                    } while (!(ga && gb && gc));
+                    prv[s].z = a; prv[s].v = b2; prv[s].la = c2;
+                }
+            }
+        }
+        __syncthreads();
+        // ---- steps 5-7; every thread of every CTA decides from the same bits ----
+        const double c = red[32 + par], c_prev = red[32 + (par ^ 1)];
+        it_done = it + 1;
+        const bool stop = p.tol > 0.0 && c < p.tol;
+        const bool accept = !stop && c <= p.eta * c_prev;
+        if (!accept && !stop) ++restarts;
+        if (cta == 0 && tid == 0 && p.hist_c && it < p.hist_cap) { p.hist_c[it] = c; p.hist_a[it] = (unsigned char)accept; }
+        if (stop) { done = true; return true; }
+        if (accept) {
+            kap = jacc < C::KAPN ? sKap[jacc] : (T)kappa_tab[jacc];
+            ++jacc;
+        } else {
+            kap = (T)0; jacc = 0;
+        }
+        return false;
+    };
+
+    bool in_b = false;                           // which of (sa, sb) holds the current iterate
+    for (int it = 0; it < iters; it += 2) {
+        if (iteration(sa, sb, it, 0)) { in_b = true; break; }
+        in_b = true;
+        if (it + 1 >= iters) break;
+        if (iteration(sb, sa, it + 1, 1)) { in_b = false; break; }
+        in_b = false;
+    }
+    // ---- results: iterate -> S[i_cur], xbar and Delta u of the last iteration, control block ----
+#pragma unroll
+    for (int s = 0; s < SPG; ++s) {
+        if (in_b) sa[s] = sb[s];                 // register moves; a reference select would force local memory
+        if (!(real[s] && rowok)) continue;
+        const int k = k0 - 1 + s * ngroups + g;
+        T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(0, k);
+        rec[p.oZ() + li] = sa[s].z; rec[p.oV() + li] = sa[s].v; rec[p.oTH() + li] = sa[s].th;
+        rec[p.oBE() + li] = sa[s].be; rec[p.oLA() + li] = sa[s].la;
+        p.X[(size_t)k * NB + li] = blkp[s][OX + li];
+        if (li >= NX) {
+            p.DU[(size_t)k * NU + (li - NX)] = blkp[s][ODU + li - NX];
+            if (DU) { rec[p.oD() + (li - NX)] = sa[s].d; rec[p.oDE() + (li - NX)] = sa[s].de; }
+        }
+    }
+    if (cta == 0 && tid == 0) {
+        InstCtl c = p.ctl[0];
+        const int last = (it_done - 1) & 1;
+        c.alpha = alpha_tab[jacc]; c.c_last = it_done ? red[32 + last] : p.c0;
+        c.c_prev = done ? red[32 + (last ^ 1)] : c.c_last;
+        c.kappa = (double)kap;
+        c.done = done ? 1 : 0; c.iters = it_done; c.restarts = restarts;
+        p.ctl[0] = c;
+    }
+}
+
+struct CoopPlan { int grid, spg, threads, slots; size_t smem; };
+
+int env_int_o(const char *name, int dflt)
+{
+    const char *v = getenv(name);
+    return v && *v ? atoi(v) : dflt;
+}
+
+template <typename T, int NX, int NU>
+bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
+{
+    using C = OCfg<T, NX, NU>;
+    const int gmax = std::min(h->sm_count, 32 * C::MAXJ);
+    int grid = std::min(h->N, gmax);
+    const int gforce = env_int_o("PIMPC_COOP_GRID", 0);        // test hook: fewer CTAs = longer ranges per CTA
+    if (gforce > 0) grid = std::min(grid, gforce);
+    const int L = (h->N + grid - 1) / grid;                    // longest range
+    const int slots = L + 2, gpw = 32 / C::LPS;
+    const int spg_max = sizeof(T) == 8 ? 1 : 2;
+    int spg = std::min(spg_max, std::max(1, env_int_o("PIMPC_COOP_SPG", 1)));   // test hook: stages per lane group
+    while (spg <= spg_max && ((slots + spg - 1) / spg + gpw - 1) / gpw > 31) ++spg;
+    if (spg > spg_max) { if (why) *why = "horizon too long for the register-resident iterates of the COOP engine"; return false; }
+    const int ncw = ((slots + spg - 1) / spg + gpw - 1) / gpw;
+    const size_t smem = C::smem_bytes(slots);
+    if (smem > h->smem_optin) { if (why) *why = "stage matrices of a CTA's range do not fit in shared memory"; return false; }
+    pl->grid = grid; pl->spg = spg; pl->threads = (ncw + 1) * 32; pl->slots = slots; pl->smem = smem;
+    return true;
+}
+
+template <typename T, int NX, int NU, int SPG, int MAXT>
+int launch_coop(pimpc_s *h, int iters, double tol, const CoopPlan &pl)
+{
+    using C = OCfg<T, NX, NU>;
+    typedef typename Tagged<double>::W PW;
+    typedef typename Tagged<T>::W HW;
+    auto kern = h->has_du ? k_coop<T, NX, NU, SPG, MAXT, true> : k_coop<T, NX, NU, SPG, MAXT, false>;
+    PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    int occ = 0;
+    PIMPC_CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, pl.smem));
+    if (occ < 1) { h->errmsg = "COOP kernel does not fit on an SM"; return PIMPC_EINVAL; }
+    const size_t pbytes = 2 * (size_t)pl.grid * sizeof(PW), hbytes = 2 * (size_t)pl.grid * C::HALO * sizeof(HW);
+    const size_t need = pbytes + hbytes;
+    if (h->coop_bytes < need) {
+        if (h->coop_buf) { cudaFree(h->coop_buf); h->device_bytes -= h->coop_bytes; h->coop_buf = nullptr; h->coop_bytes = 0; }
+        if (cudaMalloc(&h->coop_buf, need) != cudaSuccess) { cudaGetLastError(); h->errmsg = "cudaMalloc (COOP exchange) failed"; return PIMPC_ENOMEM; }
+        h->coop_bytes = need; h->device_bytes += need;
+    }
+    PIMPC_CUDA_TRY(h, cudaMemsetAsync(h->coop_buf, 0, need, h->stream));       // tag 0 = nothing published yet
+    Prob<T> p = make_prob<T>(h, tol);
+    PW *part = (PW *)h->coop_buf;
+    HW *halo = (HW *)((unsigned char *)h->coop_buf + pbytes);
+    const double *at = h->alpha_tab, *kt = h->kappa_tab;
+    void *args[] = {(void *)&p, (void *)&at, (void *)&kt, (void *)&iters, (void *)&part, (void *)&halo};
+    PIMPC_CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)kern, dim3(pl.grid), dim3(pl.threads), args, pl.smem, h->stream));
+    h->info.grid = pl.grid; h->info.block = pl.threads; h->info.smem_bytes = pl.smem;
+    return 1;
+}
+
+template <typename T, int NX, int NU>
+int run_coop_t(pimpc_s *h, int iters, double tol)
+{
+    CoopPlan pl;
+    std::string why;
+    if (!plan_coop<T, NX, NU>(h, &pl, &why)) { h->errmsg = "COOP engine not applicable: " + why; return PIMPC_EINVAL; }
+    int launches = ensure_alpha_table(h, iters);
+    if (launches < 0) return launches;
+    int n;
+    // thread ceilings: the register budget per thread follows from the block size actually needed
+    if constexpr (sizeof(T) == 8) {
+        n = pl.threads <= 384 ? launch_coop<T, NX, NU, 1, 384>(h, iters, tol, pl)
+            : pl.threads <= 512 ? launch_coop<T, NX, NU, 1, 512>(h, iters, tol, pl)
+                                : launch_coop<T, NX, NU, 1, 1024>(h, iters, tol, pl);
+    } else if (pl.spg == 1) {
+        n = pl.threads <= 512 ? launch_coop<T, NX, NU, 1, 512>(h, iters, tol, pl) : launch_coop<T, NX, NU, 1, 1024>(h, iters, tol, pl);
+    } else {
+        n = pl.threads <= 640 ? launch_coop<T, NX, NU, 2, 640>(h, iters, tol, pl) : launch_coop<T, NX, NU, 2, 1024>(h, iters, tol, pl);
+    }
+    return n < 0 ? n : n + launches;
+}
+
+bool coop_shape(const pimpc_s *h) { return (h->nx == 12 && h->nu == 4) || (h->nx == 4 && h->nu == 2); }
+
+} // namespace
+
+bool coop_supported(const pimpc_s *h, std::string *why)
+{
+    if (h->batch != 1) { if (why) *why = "COOP engine is for batch = 1"; return false; }
+    if (!coop_shape(h)) { if (why) *why = "no COOP instantiation for this (nx, nu)"; return false; }
+    if (h->bnd_per_instance || h->cost_per_instance) { /* batch = 1: strides are irrelevant */ }
+    CoopPlan pl;
+    const bool d = h->dtype == PIMPC_F64;
+    if (h->nx == 12) return d ? plan_coop<double, 12, 4>(h, &pl, why) : plan_coop<float, 12, 4>(h, &pl, why);
+    return d ? plan_coop<double, 4, 2>(h, &pl, why) : plan_coop<float, 4, 2>(h, &pl, why);
+}
+
+int run_coop(pimpc_s *h, int iters, double tol)
+{
+    std::string why;
+    if (!coop_supported(h, &why)) { h->errmsg = "COOP engine not applicable: " + why; return PIMPC_EINVAL; }
+    const bool d = h->dtype == PIMPC_F64;
+    if (h->nx == 12) return d ? run_coop_t<double, 12, 4>(h, iters, tol) : run_coop_t<float, 12, 4>(h, iters, tol);
+    return d ? run_coop_t<double, 4, 2>(h, iters, tol) : run_coop_t<float, 4, 2>(h, iters, tol);
+}

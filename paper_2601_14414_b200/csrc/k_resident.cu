@@ -405,10 +405,8 @@ bool resident_supported(const pimpc_s *h, std::string *why)
     return true;
 }
 
-int run_resident(pimpc_s *h, int iters, double tol)
+int ensure_alpha_table(pimpc_s *h, int iters)
 {
-    ResidentPlan pl;
-    if (!plan_for(h, &pl) || h->N > pl.max_stages) { h->errmsg = "RESIDENT engine not applicable"; return PIMPC_EINVAL; }
     int launches = 0;
     if (h->tab_cap < iters + 2) {
         if (h->alpha_tab) { cudaFree(h->alpha_tab); cudaFree(h->kappa_tab); h->alpha_tab = h->kappa_tab = nullptr; }
@@ -421,6 +419,15 @@ int run_resident(pimpc_s *h, int iters, double tol)
         h->tab_cap = cap;
         ++launches;
     }
+    return launches;
+}
+
+int run_resident(pimpc_s *h, int iters, double tol)
+{
+    ResidentPlan pl;
+    if (!plan_for(h, &pl) || h->N > pl.max_stages) { h->errmsg = "RESIDENT engine not applicable"; return PIMPC_EINVAL; }
+    const int launches = ensure_alpha_table(h, iters);
+    if (launches < 0) return launches;
     const int nwarps = (h->N + pl.spw - 1) / pl.spw;
     int n;
     if (h->dtype == PIMPC_F32 && h->nx == 12) {

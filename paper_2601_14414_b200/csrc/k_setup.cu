@@ -99,6 +99,136 @@ __global__ void __launch_bounds__(256) k_setup(Prob<T> p)
     else if (!ok && tid == 0) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
 }
 
+// ---- a0 for small stages (nb <= 32): one lane per matrix row, a group of LPS lanes per (instance, stage) --------
+// Row i of the SPD matrix lives in the registers of lane i (double precision whatever the dtype); the pivot
+// row of each Gauss-Jordan exchange step is broadcast through a per-group shared-memory row.  Same arithmetic
+// as gj_invert above (no pivoting; safe for SPD), ~40 x less time than one CTA per stage on 16 x 16 blocks.
+__host__ __device__ constexpr int pow2ceil_k(int v) { int p = 1; while (p < v) p <<= 1; return p; }
+
+template <int W, int NPIV>
+__device__ __forceinline__ bool gj_rows(double (&S)[W], double *rowb, const int li)
+{
+    bool ok = true;
+#pragma unroll
+    for (int p = 0; p < NPIV; ++p) {
+        __syncwarp();
+        if (li == p) {
+#pragma unroll
+            for (int j = 0; j < W; ++j) rowb[j] = S[j];
+        }
+        __syncwarp();
+        const double piv = rowb[p], colv = S[p];
+        if (!(piv > 0.0) || !isfinite(piv)) ok = false;
+        const double inv = 1.0 / piv;
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const double r = rowb[j];
+            double v;
+            if (li == p) v = (j == p) ? inv : r * inv;
+            else v = (j == p) ? -colv * inv : S[j] - colv * r * inv;
+            S[j] = v;
+        }
+    }
+    __syncwarp();
+    return ok;
+}
+
+template <typename T, int NX, int NU>
+__global__ void __launch_bounds__(128) k_setup_small(Prob<T> p)
+{
+    constexpr int NB = NX + NU, LPS = pow2ceil_k(NB), SPW = 32 / LPS, GPB = 4 * SPW, TS = LPS + 1;
+    constexpr int GSZ = (NX * LPS > LPS * TS ? NX * LPS : LPS * TS) + LPS;
+    __shared__ double sm[GPB * GSZ];
+    const int tid = threadIdx.x, g = tid / LPS, li = tid % LPS, N = p.N;
+    const long long nst = (long long)p.batch * N, sraw = (long long)blockIdx.x * GPB + g;
+    const bool act = sraw < nst;
+    const long long sidx = act ? sraw : nst - 1;               // idle groups repeat the last stage and do not store
+    const int b = (int)(sidx / N), k = (int)(sidx - (long long)b * N);
+    double *buf = sm + g * GSZ, *rowb = buf + (GSZ - LPS);
+    const bool last = (k == N - 1), rowok = li < NB;
+    const T *A1 = p.A + (sidx + (last ? 0 : 1)) * NX * NX, *B1 = p.B + (sidx + (last ? 0 : 1)) * NX * NU;
+    const T *Ak = p.A + sidx * NX * NX, *Bk = p.B + sidx * NX * NU;
+    const T *Qx = (last && p.P) ? p.P + (size_t)b * p.cost_stride_q : p.Q + (size_t)b * p.cost_stride_q;
+    const T *Rx = p.R + (size_t)b * p.cost_stride_r;
+    const double rho = p.rho;
+    bool finite = true;
+
+    // H_k = (Qbar + rho I + rho Abar_{k+1}^T Abar_{k+1})^-1, k < N-1;  (Qbar_N + rho I)^-1, k = N-1
+#pragma unroll
+    for (int r = 0; r < NX; ++r) {                             // [A_{k+1} B_{k+1}] as doubles, column li by lane li
+        const double a1 = li < NX ? (double)A1[r * NX + li] : (rowok ? (double)B1[r * NU + (li - NX)] : 0.0);
+        const double a0 = li < NX ? (double)Ak[r * NX + li] : (rowok ? (double)Bk[r * NU + (li - NX)] : 0.0);
+        if (!isfinite(a1) || !isfinite(a0)) finite = false;
+        buf[r * LPS + li] = a1;
+    }
+    __syncwarp();
+    double S[LPS];
+    {
+        double acc[LPS];
+#pragma unroll
+        for (int j = 0; j < LPS; ++j) acc[j] = (j == li && li >= NX) ? 1.0 : 0.0;      // the [0 I] rows of Abar
+#pragma unroll
+        for (int r = 0; r < NX; ++r) {
+            const double ai = buf[r * LPS + li];
+#pragma unroll
+            for (int j = 0; j < LPS; ++j) acc[j] += ai * buf[r * LPS + j];
+        }
+#pragma unroll
+        for (int j = 0; j < LPS; ++j) {
+            double s = 0.0;
+            if (rowok && j < NB) {
+                if (li < NX && j < NX) s = (double)Qx[li * NX + j];
+                else if (li >= NX && j >= NX) s = (double)Rx[(li - NX) * NU + (j - NX)];
+                if (j == li) s += rho;
+                if (!last) s += rho * acc[j];
+            } else if (j == li) s = 1.0;                        // pad rows: identity
+            if (!isfinite(s)) finite = false;
+            S[j] = s;
+        }
+    }
+    bool ok = gj_rows<LPS, NB>(S, rowb, li);
+#pragma unroll
+    for (int j = 0; j < LPS; ++j) buf[li * TS + j] = S[j];
+    __syncwarp();
+    if (act && rowok) {
+        T *Hk = p.H + (size_t)sidx * NB * NB + (size_t)li * NB;
+#pragma unroll
+        for (int j = 0; j < NB; ++j) Hk[j] = (T)(0.5 * (S[j] + buf[j * TS + li]));      // exactly symmetric
+    }
+    __syncwarp();
+
+    // M_k = (B_k^T B_k + I [+ Wdu/rho] [+ I])^-1  so that J_k = M_k Bbar_k^T  (R12, R13)
+    constexpr int MW = NU;
+    for (int idx = li; idx < NX * NU; idx += LPS) buf[idx] = (double)Bk[idx];
+    __syncwarp();
+    double Mr[MW];
+#pragma unroll
+    for (int j = 0; j < MW; ++j) {
+        double s = (j == li) ? 1.0 : 0.0;
+        if (li < NU) {
+            for (int r = 0; r < NX; ++r) s += buf[r * NU + li] * buf[r * NU + j];
+            if (p.Wdu) s += (double)p.Wdu[(size_t)b * p.cost_stride_r + li * NU + j] / rho;
+            if (p.has_du && j == li) s += 1.0;
+        }
+        if (!isfinite(s)) finite = false;
+        Mr[j] = s;
+    }
+    ok = gj_rows<MW, NU>(Mr, rowb, li) && ok;
+    __syncwarp();
+    if (li < NU) {
+#pragma unroll
+        for (int j = 0; j < MW; ++j) buf[li * TS + j] = Mr[j];
+    }
+    __syncwarp();
+    if (act && li < NU) {
+        T *Mk = p.M + (size_t)sidx * NU * NU + (size_t)li * NU;
+#pragma unroll
+        for (int j = 0; j < MW; ++j) Mk[j] = (T)(0.5 * (Mr[j] + buf[j * TS + li]));
+    }
+    if (!finite) atomicOr(p.err, PIMPC_DEVERR_NONFINITE);
+    else if (!ok) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
+}
+
 // Input of Alg. 1: hats = iterates (i_prev = i_cur), alpha_0 = 1, c^0 = c0.
 template <typename T>
 __global__ void k_begin(Prob<T> p)
@@ -213,9 +343,22 @@ Prob<T> make_prob(pimpc_s *h, double tol)
 template Prob<float> make_prob<float>(pimpc_s *, double);
 template Prob<double> make_prob<double>(pimpc_s *, double);
 
+template <typename T, int NX, int NU>
+static int setup_small_t(pimpc_s *h)
+{
+    Prob<T> p = make_prob<T>(h, 0.0);
+    constexpr int GPB = 4 * (32 / pow2ceil_k(NX + NU));
+    const long long nst = (long long)h->batch * h->N;
+    k_setup_small<T, NX, NU><<<(unsigned)((nst + GPB - 1) / GPB), 128, 0, h->stream>>>(p);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 1;
+}
+
 template <typename T>
 static int setup_t(pimpc_s *h)
 {
+    if (h->nx == 12 && h->nu == 4) return setup_small_t<T, 12, 4>(h);
+    if (h->nx == 4 && h->nu == 2) return setup_small_t<T, 4, 2>(h);
     Prob<T> p = make_prob<T>(h, 0.0);
     const size_t smem = ((size_t)h->nb * h->nb + 2 * h->nb) * sizeof(double);
     if (smem > 48 * 1024)

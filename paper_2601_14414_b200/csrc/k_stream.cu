@@ -64,6 +64,7 @@ struct LInst {
     float kappa_f; int pad0;
     double kappa;
     int b, i_prev, i_cur, i_new, done, iters, restarts, owner;
+    int c_lo, c_hi;                                        // first / last CTA whose range holds a dual step of the instance
 };
 
 struct Seg { int b, j0, nsteps, pstep, halo; };   // steps j0..: optional P step (state of stage j0 only), then S steps
@@ -145,7 +146,7 @@ struct Cursor {
 
 template <typename T, int NX, int NU>
 __global__ void __launch_bounds__(SCfg<T, NX, NU>::NT)
-k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ partial, const int iters, const int nslot)
+k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ partial, const int iters, const int nslot, const int span)
 {
     using C = SCfg<T, NX, NU>;
     constexpr int NB = C::NB, IP = C::IP, NPART = C::NPART, REC = C::REC, BLOB = C::BLOB, SLOT = C::SLOT;
@@ -181,6 +182,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
         L.b = b; L.i_prev = c.i_prev; L.i_cur = c.i_cur; L.i_new = c.i_new; L.done = c.done; L.iters = 0; L.restarts = 0;
         const long long first = (long long)b * N1;
         L.owner = first >= s0 && first < s1;
+        L.c_lo = (int)(((first + 1) * G - 1) / S_tot); L.c_hi = (int)(((first + N1) * G - 1) / S_tot);
     }
     __syncthreads();
     uint32_t phase = 0;                                    // parity bit per ring slot
@@ -422,7 +424,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                 if (tid == 0) {
                     double t = 0.0;
                     for (int w = 0; w < C::NW; ++w) t += sm.red[w];
-                    partial[(size_t)cta * C::MAXI + li] = t;
+                    partial[(size_t)L.b * span + ((int)cta - L.c_lo)] = t;     // slot = position among the instance's CTAs
                 }
                 acc = 0.0;
             }
@@ -433,15 +435,16 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
         fence_proxy_async();
         grid.sync();
         // ---- steps 4-7: c of every instance of the range, same order in every CTA ----
-        if (tid < n_local && !sm.inst[tid].done) {
-            LInst &L = sm.inst[tid];
-            const long long base = (long long)L.b * N1;
-            const long long c_lo = ((base + 1) * G - 1) / S_tot, c_hi = ((base + N1) * G - 1) / S_tot;
+        // one warp per instance: lanes stride over the instance's CTAs, then a fixed butterfly (bit-identical in every CTA)
+        for (int li = warp; li < n_local; li += C::NW) {
+            LInst &L = sm.inst[li];
+            if (L.done) continue;
+            const double *pp = partial + (size_t)L.b * span;
             double s = 0.0;
-            for (long long c2 = c_lo; c2 <= c_hi; ++c2) {
-                const int bf = (int)((c2 * S_tot / G) / N1);
-                s += __ldcg(&partial[(size_t)c2 * C::MAXI + (L.b - bf)]);
-            }
+            for (int q = lane; q <= L.c_hi - L.c_lo; q += 32) s += __ldcg(&pp[q]);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane != 0) continue;
             const double c = p.rho * s;
             L.c_last = c; L.iters = it + 1;
             int accept = 0;
@@ -467,7 +470,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
         __syncthreads();
         // partial[] is rewritten next iteration: every CTA must have read it first.  The next grid barrier
         // comes only after the next writes, so double-buffer by iteration parity instead of a second barrier.
-        partial += (it & 1) ? -(ptrdiff_t)(gridDim.x * C::MAXI) : (ptrdiff_t)(gridDim.x * C::MAXI);
+        partial += (it & 1) ? -(ptrdiff_t)((size_t)p.batch * span) : (ptrdiff_t)((size_t)p.batch * span);
     }
     if (tid < n_local && sm.inst[tid].owner) {
         const LInst &L = sm.inst[tid];
@@ -541,7 +544,8 @@ int run_stream_t(pimpc_s *h, int iters, double tol)
         if (cudaMalloc(&h->blob, bbytes) != cudaSuccess) { cudaGetLastError(); h->errmsg = "cudaMalloc (stage blobs) failed"; return PIMPC_ENOMEM; }
         h->blob_bytes = bbytes; h->device_bytes += bbytes; h->blob_dirty = true;
     }
-    const size_t pneed = 2 * (size_t)pl.grid * C::MAXI;
+    int span = (pl.grid + h->batch - 1) / h->batch + 2;        // CTAs whose ranges can touch one instance
+    const size_t pneed = 2 * (size_t)h->batch * span;
     if (h->spartial_cap < pneed) {
         if (h->spartial) cudaFree(h->spartial);
         PIMPC_CUDA_TRY(h, cudaMalloc(&h->spartial, pneed * sizeof(double)));
@@ -557,7 +561,7 @@ int run_stream_t(pimpc_s *h, int iters, double tol)
     const T *blob = (const T *)h->blob;
     double *partial = h->spartial;
     int nslot = pl.nslot;
-    void *args[] = {(void *)&p, (void *)&blob, (void *)&partial, (void *)&iters, (void *)&nslot};
+    void *args[] = {(void *)&p, (void *)&blob, (void *)&partial, (void *)&iters, (void *)&nslot, (void *)&span};
     PIMPC_CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)k_stream<T, NX, NU>, dim3(pl.grid), dim3(C::NT), args, pl.smem, h->stream));
     h->info.grid = pl.grid; h->info.block = C::NT; h->info.smem_bytes = pl.smem;
     return launches + 1;

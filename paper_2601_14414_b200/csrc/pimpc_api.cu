@@ -239,7 +239,7 @@ int pimpc_destroy(pimpc_t h)
     if (!h->poisoned) cudaStreamSynchronize(h->stream);
     void *ptrs[] = {h->A, h->B, h->e, h->x0, h->uprev, h->Q, h->R, h->P, h->Wdu, h->qbar, h->lo, h->hi, h->dlo, h->dhi,
                     h->H, h->M, h->S, h->X, h->DU, h->ctl, h->partial, h->hist_c, h->hist_a, h->err,
-                    h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab, h->spartial};
+                    h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab, h->spartial, h->coop_buf};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (auto &e : h->ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();
@@ -386,16 +386,18 @@ int pimpc_solve(pimpc_t h, int max_iters, double tol)
     std::string why;
     if (engine == PIMPC_ENGINE_AUTO)
         engine = resident_supported(h, &why) ? PIMPC_ENGINE_RESIDENT
+                 : coop_supported(h, &why) ? PIMPC_ENGINE_COOP
                  : (stream_supported(h, &why) ? PIMPC_ENGINE_STREAM : PIMPC_ENGINE_STAGED);
     if (engine == PIMPC_ENGINE_RESIDENT && !resident_supported(h, &why))
         return fail(h, PIMPC_EINVAL, "RESIDENT engine not applicable: " + why);
     if (engine == PIMPC_ENGINE_STREAM && !stream_supported(h, &why))
         return fail(h, PIMPC_EINVAL, "STREAM engine not applicable: " + why);
-    if (engine == PIMPC_ENGINE_COOP)
-        return fail(h, PIMPC_EINVAL, "engine not available in this build");
+    if (engine == PIMPC_ENGINE_COOP && !coop_supported(h, &why))
+        return fail(h, PIMPC_EINVAL, "COOP engine not applicable: " + why);
     if (max_iters > 0) {
         if (engine == PIMPC_ENGINE_RESIDENT) n = run_resident(h, max_iters, tol);
         else if (engine == PIMPC_ENGINE_STREAM) n = run_stream(h, max_iters, tol);
+        else if (engine == PIMPC_ENGINE_COOP) n = run_coop(h, max_iters, tol);
         else n = run_staged(h, max_iters, tol);
         if (n < 0) return n;
         launches += n;

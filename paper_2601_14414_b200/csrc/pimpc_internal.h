@@ -93,6 +93,8 @@ struct pimpc_s {
     double *spartial = nullptr;              // [2][grid][MAXI] partial sums of c of the STREAM engine
     size_t spartial_cap = 0;
     bool blob_dirty = true;
+    void *coop_buf = nullptr;                // tagged exchange words of the COOP engine (partials of c, boundary iterates)
+    size_t coop_bytes = 0;
 
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // before cache kernel, before iteration, after iteration
     bool ev_pending = false, ev_setup = false;
@@ -112,6 +114,9 @@ int launch_begin(pimpc_s *h);                       // Alg. 1 input: alpha=1, c_
 int run_staged(pimpc_s *h, int iters, double tol);  // v0 engine
 int run_resident(pimpc_s *h, int iters, double tol);
 bool resident_supported(const pimpc_s *h, std::string *why);
+int ensure_alpha_table(pimpc_s *h, int iters);     // alpha_j / kappa_j tables cover `iters` accepted steps; returns launches
+int run_coop(pimpc_s *h, int iters, double tol);
+bool coop_supported(const pimpc_s *h, std::string *why);
 int run_stream(pimpc_s *h, int iters, double tol);
 bool stream_supported(const pimpc_s *h, std::string *why);
 int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res_dev);

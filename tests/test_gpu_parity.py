@@ -169,6 +169,62 @@ def test_stream_engine_early_stop_and_warm_start(oracle, pimpc, stream_grid, gri
         assert parity.relerr(z2[b], o.Z) <= 1e-9
 
 
+# ---- COOP engine (batch 1, horizon spread over the SMs, tagged-word exchange instead of grid barriers) ------
+@pytest.fixture
+def coop_env(monkeypatch):
+    def set_(grid=0, spg=0):
+        for name, v in (("PIMPC_COOP_GRID", grid), ("PIMPC_COOP_SPG", spg)):
+            if v:
+                monkeypatch.setenv(name, str(v))
+            else:
+                monkeypatch.delenv(name, raising=False)
+    return set_
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("grid", [0, 1, 2, 7])
+@pytest.mark.parametrize("shape", [(12, 4, 41), (4, 2, 23), (12, 4, 150), (4, 2, 1), (12, 4, 2)])
+def test_coop_engine_all_options(oracle, pimpc, coop_env, shape, grid, dtype):
+    """grid = 0: one stage per CTA while N <= 148 (every stage has two ghosts); 1: a single CTA, no exchange;
+    2, 7: ragged ranges.  All optional terms on."""
+    nx, nu, N = shape
+    coop_env(grid)
+    p = wl.random_ltv(nx, nu, N, 1, seed=nx * 10 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
+                      qbar=True, bounds=0.8, du_bound=0.5)
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="coop", iters=120, tol=0.0)
+    assert g["info"]["engine"] == pimpc.ENGINE_COOP
+    parity.check_properties(p, dtype, g)
+
+
+@pytest.mark.parametrize("grid", [3, 0])
+def test_coop_engine_two_stages_per_group_fp32(oracle, pimpc, coop_env, grid):
+    coop_env(grid, spg=2)
+    p = wl.random_ltv(12, 4, 100, 1, seed=5, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f32", engine="coop", iters=150, tol=0.0)
+    assert g["info"]["engine"] == pimpc.ENGINE_COOP
+
+
+@pytest.mark.parametrize("grid", [0, 5])
+def test_coop_engine_unbounded_plain_admm_early_stop_warm_start(oracle, pimpc, coop_env, grid):
+    coop_env(grid)
+    p = wl.random_ltv(4, 2, 9, 1, seed=77, affine=True, bounds=None, du_bound=None)
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="coop", iters=300, tol=0.0)
+    assert "D" not in g
+    p = wl.quadrotor_ltv(12, 1, iters=120, tol=0.0)
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="coop", eta=0.0)
+    assert np.all(g["res"]["restarts"] == 120)
+    p = wl.quadrotor_ltv(10, 1, iters=2000, tol=1e-4, rho=10.0, name="C2-tol")
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="coop")
+    assert int(g["res"]["converged"][0]) == 1 and int(g["res"]["iters"][0]) < 2000
+    p = wl.quadrotor_ltv(30, 1, iters=40, tol=0.0)
+    s = pimpc.Solver(p.nx, p.nu, p.N, 1, dtype="f64", engine="coop")
+    s.set_problem(p); s.solve(40)
+    warm = {k: s.get_state(k) for k in ("Z", "V", "TH", "BE", "LA", "D", "DE")}
+    s.solve(25)
+    o = parity.oracle_run(oracle, p, "f64", 0, iters=25, tol=0.0, warm=warm)
+    assert parity.relerr(s.get_state("Z")[0], o.Z) <= 1e-9
+
+
 # ---- odd shapes, optional terms, edge cases -----------------------------------------------------
 @pytest.mark.parametrize("engine", ENGINES_SMALL)
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
