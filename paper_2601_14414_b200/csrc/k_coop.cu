@@ -16,6 +16,7 @@
 //     neighbour's next partial first.
 // The launch is cooperative only to guarantee co-residency of the polling CTAs.
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 
 #include "pimpc_internal.h"
@@ -93,9 +94,23 @@ struct OCfg {
     // exchange buffers per CTA and parity (tagged words): to the left neighbour (z, v, lambda) of the first stage,
     // to the right neighbour (z, theta) of the last stage
     static constexpr int HALO = 5 * LPS;
+    // every partial of c sits in its own 256-byte granule: the polls of all CTAs spread over the L2 slices
+    static constexpr int PSTRIDE = 16;                         // in 16-byte tagged words
+    // replicas of the broadcast c; largest all-to-all grid.  Measured on B200 inside this kernel (C3, N = 1000, 148 CTAs):
+    // all-to-all 3.2 us/iteration, gather + broadcast 4.0 us/iteration, so the two-hop path is kept for grids > 160 only.
+    static constexpr int NREP = 8, A2A_MAX = 160;
 };
 
 template <typename T> struct OState { T z, v, th, be, la, d, de; };
+
+// Developer aid (off by default): -DPIMPC_COOP_PROF accumulates clock64() per phase in CTA 0 and prints the means.
+#ifdef PIMPC_COOP_PROF
+#define PROF_DECL long long prof_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, prof_last = clock64();
+#define PROF_MARK(i) { const long long t_ = clock64(); prof_t[i] += t_ - prof_last; prof_last = t_; }
+#else
+#define PROF_DECL
+#define PROF_MARK(i)
+#endif
 
 template <typename T, int NX, int NU, int SPG, int MAXT, bool DU>
 __global__ void __launch_bounds__(MAXT, 1)
@@ -190,6 +205,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     int jacc = 0, it_done = 0, restarts = 0;
     bool done = false;
     __syncthreads();
+    PROF_DECL
 
     // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.  par = it & 1.
     auto iteration = [&](OState<T> (&cur)[SPG], OState<T> (&prv)[SPG], const int it, const int par) -> bool {
@@ -213,7 +229,9 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             if (has_e && exist[s]) { ev[s] = blkp[s][OE + li]; w -= ev[s]; }
             if (exist[s]) { blkp[s][OW + li] = w; blkp[s][OD + li] = dv[s]; }
         }
+        PROF_MARK(0)
         __syncthreads();
+        PROF_MARK(1)
         // ---- B: step 1: g = Abar_{k+1}^T w_{k+1}, h_k; rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat] ----
 #pragma unroll
         for (int s = 0; s < SPG; ++s) {
@@ -274,7 +292,9 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 if (ulane) blkp[s][ODU + li - NX] = du[s];
             }
         }
+        PROF_MARK(2)
         __syncthreads();
+        PROF_MARK(3)
         // ---- D: steps 2-4 of the real stages ----
         T acc = (T)0;
 #pragma unroll
@@ -335,30 +355,41 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 #pragma unroll
         for (int o = 16; o >= LPS; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
         if (lane == 0 && !comm) red[warp] = sum;
+        PROF_MARK(4)
         __syncthreads();
+        PROF_MARK(5)
         if (comm) {
             sum = lane < ncw ? red[lane] : 0.0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            typename TD::W *pp = part + (size_t)par * G;
-            if (lane == 0) TD::st(pp + cta, sum, tag);
-            double vals[C::MAXJ];
-            bool got[C::MAXJ];
+            // small grids: every CTA polls every partial (one hop).  Large grids: CTA 0 gathers, sums and publishes c
+            // in NREP replicas, the others poll one replica (two hops, but 148 x 148 polls would take longer).
+            typename TD::W *pp = part + (size_t)par * (G + C::NREP) * C::PSTRIDE;
+            if (lane == 0) TD::st(pp + (size_t)cta * C::PSTRIDE, sum, tag);
+            const bool a2a = G <= C::A2A_MAX;
+            if (a2a || cta == 0) {
+                double vals[C::MAXJ];
+                bool got[C::MAXJ];
 #pragma unroll
-            for (int u = 0; u < C::MAXJ; ++u) { vals[u] = 0.0; got[u] = lane + 32 * u >= G; }
-            bool all;
-            do {
-                all = true;
+                for (int u = 0; u < C::MAXJ; ++u) { vals[u] = 0.0; got[u] = lane + 32 * u >= G; }
+                bool all;
+                do {
+                    all = true;
 #pragma unroll
-                for (int u = 0; u < C::MAXJ; ++u) {
-                    if (!got[u]) { got[u] = TD::ld(pp + lane + 32 * u, tag, vals[u]); all = all && got[u]; }
-                }
-            } while (!all);
-            sum = 0.0;
+                    for (int u = 0; u < C::MAXJ; ++u) {
+                        if (!got[u]) { got[u] = TD::ld(pp + (size_t)(lane + 32 * u) * C::PSTRIDE, tag, vals[u]); all = all && got[u]; }
+                    }
+                } while (!all);
+                sum = 0.0;
 #pragma unroll
-            for (int u = 0; u < C::MAXJ; ++u) sum += vals[u];
+                for (int u = 0; u < C::MAXJ; ++u) sum += vals[u];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+                if (!a2a && lane < C::NREP) TD::st(pp + (size_t)(G + lane) * C::PSTRIDE, sum, tag);
+            } else {
+                if (lane == 0) while (!TD::ld(pp + (size_t)(G + cta % C::NREP) * C::PSTRIDE, tag, sum)) {}
+                sum = __shfl_sync(0xffffffffu, sum, 0);
+            }
             if (lane == 0) red[32 + par] = p.rho * sum;
         } else {
             // the ghosts' new iterates, published by the neighbours in their phase D of this iteration
@@ -384,7 +415,9 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 }
             }
         }
+        PROF_MARK(6)
         __syncthreads();
+        PROF_MARK(7)
         // ---- steps 5-7; every thread of every CTA decides from the same bits ----
         const double c = red[32 + par], c_prev = red[32 + (par ^ 1)];
         it_done = it + 1;
@@ -410,6 +443,12 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         if (iteration(sb, sa, it + 1, 1)) { in_b = false; break; }
         in_b = false;
     }
+#ifdef PIMPC_COOP_PROF
+    if ((cta == 0 || cta == G / 2) && (tid == 0 || tid == ncw * 32) && it_done > 0)
+        printf("coop prof cta %d tid %d: A %lld | B1 %lld | BC %lld | B2 %lld | D %lld | B3 %lld | xchg %lld | B4 %lld cycles/it\n", cta, tid,
+               prof_t[0] / it_done, prof_t[1] / it_done, prof_t[2] / it_done, prof_t[3] / it_done, prof_t[4] / it_done,
+               prof_t[5] / it_done, prof_t[6] / it_done, prof_t[7] / it_done);
+#endif
     // ---- results: iterate -> S[i_cur], xbar and Delta u of the last iteration, control block ----
 #pragma unroll
     for (int s = 0; s < SPG; ++s) {
@@ -449,7 +488,8 @@ bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
 {
     using C = OCfg<T, NX, NU>;
     const int gmax = std::min(h->sm_count, 32 * C::MAXJ);
-    int grid = std::min(h->N, gmax);
+    // ranges of >= 16 stages until 64 CTAs are busy, then as many CTAs as SMs (measured: the exchange grows with the grid)
+    int grid = std::min(gmax, std::max((h->N + 15) / 16, std::min(h->N, 64)));
     const int gforce = env_int_o("PIMPC_COOP_GRID", 0);        // test hook: fewer CTAs = longer ranges per CTA
     if (gforce > 0) grid = std::min(grid, gforce);
     const int L = (h->N + grid - 1) / grid;                    // longest range
@@ -476,7 +516,7 @@ int launch_coop(pimpc_s *h, int iters, double tol, const CoopPlan &pl)
     int occ = 0;
     PIMPC_CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, pl.smem));
     if (occ < 1) { h->errmsg = "COOP kernel does not fit on an SM"; return PIMPC_EINVAL; }
-    const size_t pbytes = 2 * (size_t)pl.grid * sizeof(PW), hbytes = 2 * (size_t)pl.grid * C::HALO * sizeof(HW);
+    const size_t pbytes = 2 * (size_t)(pl.grid + C::NREP) * C::PSTRIDE * sizeof(PW), hbytes = 2 * (size_t)pl.grid * C::HALO * sizeof(HW);
     const size_t need = pbytes + hbytes;
     if (h->coop_bytes < need) {
         if (h->coop_buf) { cudaFree(h->coop_buf); h->device_bytes -= h->coop_bytes; h->coop_buf = nullptr; h->coop_bytes = 0; }

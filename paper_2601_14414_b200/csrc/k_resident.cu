@@ -15,6 +15,7 @@
 // c is reduced in a fixed order (xor butterflies; every warp repeats the second level), so every
 // thread takes the same accept/restart decision (steps 5-7) from bit-identical numbers.
 #include <algorithm>
+#include <cstdlib>
 
 #include "pimpc_internal.h"
 
@@ -33,6 +34,17 @@ __device__ __forceinline__ void ld4(const double *p, double (&o)[4])
     o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
 }
 template <typename T> __device__ __forceinline__ T clipv(T v, T lo, T hi) { return fmin(fmax(v, lo), hi); }
+
+// (c0, c1) += (a0, a1) * (b0, b1): one packed FFMA2 on sm_100a (two IEEE fmas, half the issue slots); two DFMAs in fp64
+__device__ __forceinline__ void fma2p(float &c0, float &c1, float a0, float a1, float b0, float b1)
+{
+    const float2 r = __ffma2_rn(make_float2(a0, a1), make_float2(b0, b1), make_float2(c0, c1));
+    c0 = r.x; c1 = r.y;
+}
+__device__ __forceinline__ void fma2p(double &c0, double &c1, double a0, double a1, double b0, double b1)
+{
+    c0 = fma(a0, b0, c0); c1 = fma(a1, b1, c1);
+}
 
 // alpha_j and kappa_j after j consecutive accepted steps from alpha_0 = 1:
 // alpha_{j+1} = 0.5 + 0.5 sqrt(1 + 4 alpha_j^2), kappa_j = (alpha_j - 1) / alpha_{j+1}.
@@ -65,7 +77,7 @@ struct RCfg {
                          OC = ODU + NUP /* qbar, e, du_lo, du_hi rows */, OAT = OC + 4 * ROWP, SS0 = OAT + NX * ROWP;
     // stage stride == LPS (mod 32 words): the groups of a warp hit disjoint banks on own-element accesses
     static constexpr int SS = SS0 + ((LPS - SS0 % 32) + 32) % 32;
-    static_assert(NX % 4 == 0, "RESIDENT engine needs nx % 4 == 0");
+    static_assert(NX % 4 == 0 && NX + NUP == NBP, "RESIDENT engine needs nx % 4 == 0");
     static_assert(NX % R == 0 && LPS <= 32 && LPS >= 4 && ROWP >= NBP && ROWP % 4 == 0 && SS % 4 == 0, "bad row blocking");
     static size_t smem_bytes(int nwarps)
     {
@@ -202,7 +214,10 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                     T a4[4];
                     ld4(atp + ((r * (NX / 4) + c4 / 4) * LPS) * 4, a4);
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) { g[r][q & 1] += a4[q] * w4[q]; rd[r][q & 1] += U[r][c4 + q] * d4[q]; }
+                    for (int q = 0; q < 4; q += 2) {
+                    fma2p(g[r][0], g[r][1], a4[q], a4[q + 1], w4[q], w4[q + 1]);
+                    fma2p(rd[r][0], rd[r][1], U[r][c4 + q], U[r][c4 + q + 1], d4[q], d4[q + 1]);
+                }
                 }
             }
 #pragma unroll
@@ -217,9 +232,9 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 if (!isx[r]) own[ORH - NX + r] = rr;
             }
             __syncwarp();
-            T x[R][2], du[R];
+            T x[R][2], du2[R][2], du[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { x[r][0] = x[r][1] = (T)0; du[r] = (T)0; }
+            for (int r = 0; r < R; ++r) { x[r][0] = x[r][1] = (T)0; du2[r][0] = du2[r][1] = (T)0; }
 #pragma unroll
             for (int c4 = 0; c4 < NBP; c4 += 4) {
                 T h4[4];
@@ -227,7 +242,8 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) x[r][q & 1] += Hrow[r][c4 + q] * h4[q];   // xbar_{k+1} = H_k h_k
+                    for (int q = 0; q < 4; q += 2)                                        // xbar_{k+1} = H_k h_k
+                        fma2p(x[r][0], x[r][1], Hrow[r][c4 + q], Hrow[r][c4 + q + 1], h4[q], h4[q + 1]);
             }
 #pragma unroll
             for (int c4 = 0; c4 < NUP; c4 += 4) {
@@ -236,20 +252,22 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) if (NX + c4 + q < NBP) du[r] += U[r][NX + c4 + q] * r4[q];   // Delta u_k = M_k rhs (u-rows)
+                    for (int q = 0; q < 4; q += 2)                                        // Delta u_k = M_k rhs (u-rows)
+                        fma2p(du2[r][0], du2[r][1], U[r][NX + c4 + q], U[r][NX + c4 + q + 1], r4[q], r4[q + 1]);
             }
             T xs[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 xs[r] = x[r][0] + x[r][1];
+                du[r] = du2[r][0] + du2[r][1];
                 own[OX + r] = xs[r];
                 if (!isx[r]) own[ODU - NX + r] = du[r];
             }
             __syncthreads();
             // steps 2-4
-            T dot[R][2], avx[R];
+            T dot[R][2], av2[R][2], avx[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) { dot[r][0] = dot[r][1] = (T)0; avx[r] = (T)0; }
+            for (int r = 0; r < R; ++r) { dot[r][0] = dot[r][1] = (T)0; av2[r][0] = av2[r][1] = (T)0; }
 #pragma unroll
             for (int c4 = 0; c4 < NBP; c4 += 4) {
                 T x4[4];
@@ -257,7 +275,8 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) dot[r][q & 1] += U[r][c4 + q] * x4[q];    // [A_k B_k] xbar_k (x-rows)
+                    for (int q = 0; q < 4; q += 2)                                        // [A_k B_k] xbar_k (x-rows)
+                        fma2p(dot[r][0], dot[r][1], U[r][c4 + q], U[r][c4 + q + 1], x4[q], x4[q + 1]);
             }
 #pragma unroll
             for (int c4 = 0; c4 < NUP; c4 += 4) {
@@ -266,8 +285,11 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) if (NX + c4 + q < NBP) avx[r] += U[r][NX + c4 + q] * u4[q];  // B_k Delta u_k (x-rows)
+                    for (int q = 0; q < 4; q += 2)                                        // B_k Delta u_k (x-rows)
+                        fma2p(av2[r][0], av2[r][1], U[r][NX + c4 + q], U[r][NX + c4 + q + 1], u4[q], u4[q + 1]);
             }
+#pragma unroll
+            for (int r = 0; r < R; ++r) avx[r] = av2[r][0] + av2[r][1];
             T acc = (T)0;
 #pragma unroll
             for (int r = 0; r < R; ++r) {
@@ -301,8 +323,10 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             for (int o = 16; o >= LPS; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
             if (lane == 0) red[warp] = s;
             __syncthreads();
-            s = lane < nwarps ? red[lane] : 0.0;
             const double c_prev = red[32 + (par ^ 1)];
+            // every warp repeats the second level (butterfly over the warp partials): same bits everywhere.  A shuffle-free
+            // tree of 16 broadcast loads + DADDs per lane was measured 4 % slower on C4 (B200).
+            s = lane < nwarps ? red[lane] : 0.0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
             // steps 5-7; every thread decides from the same bits
@@ -428,9 +452,15 @@ int run_resident(pimpc_s *h, int iters, double tol)
     if (!plan_for(h, &pl) || h->N > pl.max_stages) { h->errmsg = "RESIDENT engine not applicable"; return PIMPC_EINVAL; }
     const int launches = ensure_alpha_table(h, iters);
     if (launches < 0) return launches;
-    const int nwarps = (h->N + pl.spw - 1) / pl.spw;
+    int nwarps = (h->N + pl.spw - 1) / pl.spw;
     int n;
-    if (h->dtype == PIMPC_F32 && h->nx == 12) {
+    const char *rv = getenv("PIMPC_RESIDENT_R");         // tuning hook: 1 = one row per lane (16 lanes per stage)
+    if (h->dtype == PIMPC_F32 && h->nx == 12 && !(rv && atoi(rv) == 1) && h->N <= 56) {
+        // two rows per lane, 8 lanes per stage: half the broadcast loads per FMA.  C4 on B200: 8.23 ms, against 9.11 ms
+        // with one row per lane and 8.94 ms with four
+        nwarps = (h->N + 3) / 4;
+        n = launch_resident<float, 12, 4, 2, 448>(h, iters, tol, nwarps);
+    } else if (h->dtype == PIMPC_F32 && h->nx == 12) {
         n = nwarps <= 25 ? launch_resident<float, 12, 4, 1, 800>(h, iters, tol, nwarps)
                          : launch_resident<float, 12, 4, 1, 1024>(h, iters, tol, nwarps);
     } else if (h->dtype == PIMPC_F64) {

@@ -18,7 +18,7 @@ except Exception:  # pragma: no cover
     torch = None
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpimpc.so")
+LIB_PATH = os.environ.get("PIMPC_LIB") or os.path.join(_HERE, "libpimpc.so")   # PIMPC_LIB: another build of the same ABI
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENOTPD = 0, -1, -2, -3, -4, -5
 F64, F32 = 0, 1
