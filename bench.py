@@ -235,6 +235,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--engine", default="auto")
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--only-extras", action="store_true", help="run only the C1-C3, C5 legs and print their JSON (profiling aid)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -247,6 +248,10 @@ def main():
     rank, local_rank, world = replicas.init()
     torch.cuda.set_device(local_rank)
     pk = peaks()
+    if args.only_extras:
+        if rank == 0:
+            print(json.dumps({"extras": extras(torch, pimpc, pk)}))
+        return 0
 
     lo, hi = replicas.weak_instance_range(BATCH, rank)
     prob = wl.config4(batch=BATCH, first_instance=lo)

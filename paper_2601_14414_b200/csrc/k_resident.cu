@@ -15,6 +15,7 @@
 // c is reduced in a fixed order (xor butterflies; every warp repeats the second level), so every
 // thread takes the same accept/restart decision (steps 5-7) from bit-identical numbers.
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 
 #include "pimpc_internal.h"
@@ -34,6 +35,17 @@ __device__ __forceinline__ void ld4(const double *p, double (&o)[4])
     o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
 }
 template <typename T> __device__ __forceinline__ T clipv(T v, T lo, T hi) { return fmin(fmax(v, lo), hi); }
+
+// own rows of a lane -> shared memory: one 8-byte store when a lane owns two fp32 rows
+template <typename T, int R> __device__ __forceinline__ void st_rows(T *p, const T (&v)[R])
+{
+#pragma unroll
+    for (int r = 0; r < R; ++r) p[r] = v[r];
+}
+template <> __device__ __forceinline__ void st_rows<float, 2>(float *p, const float (&v)[2])
+{
+    *reinterpret_cast<float2 *>(p) = make_float2(v[0], v[1]);
+}
 
 // (c0, c1) += (a0, a1) * (b0, b1): one packed FFMA2 on sm_100a (two IEEE fmas, half the issue slots); two DFMAs in fp64
 __device__ __forceinline__ void fma2p(float &c0, float &c1, float a0, float a1, float b0, float b1)
@@ -76,7 +88,9 @@ struct RCfg {
     static constexpr int OW = 0, OX = ROWP, OD = 2 * ROWP, OH = 3 * ROWP, ORH = 4 * ROWP, ODU = ORH + NUP,
                          OC = ODU + NUP /* qbar, e, du_lo, du_hi rows */, OAT = OC + 4 * ROWP, SS0 = OAT + NX * ROWP;
     // stage stride == LPS (mod 32 words): the groups of a warp hit disjoint banks on own-element accesses
-    static constexpr int SS = SS0 + ((LPS - SS0 % 32) + 32) % 32;
+    // (two rows per lane: 16 words, so that the 8-byte own-row accesses of a half-warp hit disjoint banks)
+    static constexpr int SST = (R == 2 && sizeof(T) == 4) ? 16 : LPS;
+    static constexpr int SS = SS0 + ((SST - SS0 % 32) + 32) % 32;
     static_assert(NX % 4 == 0 && NX + NUP == NBP, "RESIDENT engine needs nx % 4 == 0");
     static_assert(NX % R == 0 && LPS <= 32 && LPS >= 4 && ROWP >= NBP && ROWP % 4 == 0 && SS % 4 == 0, "bad row blocking");
     static size_t smem_bytes(int nwarps)
@@ -85,6 +99,15 @@ struct RCfg {
         return ((NS + 2) * SS + KAPN) * sizeof(T) + 36 * sizeof(double);
     }
 };
+
+// Developer aid (off by default): -DPIMPC_RES_PROF accumulates clock64() per phase in CTA 0 and prints the means.
+#ifdef PIMPC_RES_PROF
+#define RPROF_DECL long long prof_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, prof_last = clock64();
+#define RPROF_MARK(i) { const long long t_ = clock64(); prof_t[i] += t_ - prof_last; prof_last = t_; }
+#else
+#define RPROF_DECL
+#define RPROF_MARK(i)
+#endif
 
 template <typename T, int R>
 struct RState { T z[R], v[R], th[R], be[R], la[R], d[R], de[R]; };
@@ -170,6 +193,7 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             sBlk[OX + tid] = tid < NX ? p.x0[(size_t)b * NX + tid] : (tid < NB ? p.uprev[(size_t)b * NU + (tid - NX)] : (T)0);
         if (tid == 0) { red[32] = p.c0; red[33] = p.c0; sCnt[0] = 0; }
 
+        RPROF_DECL
         T kap = (T)0;
         int jacc = 0, it_done = 0;
         bool done = false;
@@ -179,7 +203,7 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
         // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.
         // par = it & 1 (compile-time after unrolling by two): c^{i} sits in red[32 + (par ^ 1)], c^{i+1} goes to red[32 + par].
         auto iteration = [&](RState<T, R> &cur, RState<T, R> &prv, const int it, const int par) -> bool {
-            T zh[R], vh[R], thh[R], beh[R], lah[R], dh[R], deh[R], dv[R], ev[R];
+            T zh[R], vh[R], thh[R], beh[R], lah[R], dh[R], deh[R], dv[R], ev[R], wv[R];
             // steps 6/7 of the previous iteration: hats from (cur, prev, kappa)
 #pragma unroll
             for (int r = 0; r < R; ++r) {
@@ -196,10 +220,13 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 T w = zh[r] - vh[r] + lah[r];
                 ev[r] = (T)0;
                 if (has_e) { ev[r] = own[OC + C::ROWP + r]; w -= ev[r]; }
-                own[OW + r] = w;
-                own[OD + r] = dv[r];
+                wv[r] = w;
             }
+            st_rows<T, R>(own + OW, wv);
+            st_rows<T, R>(own + OD, dv);
+            RPROF_MARK(0)
             __syncthreads();
+            RPROF_MARK(1)
             // step 1: g = Abar_{k+1}^T w_{k+1}, rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat]
             T g[R][2], rd[R][2];
 #pragma unroll
@@ -220,17 +247,20 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 }
                 }
             }
+            T hv[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 T gg = g[r][0] + g[r][1];
                 if (!isx[r]) gg += own[SS + OW + r];                                // the [0 I] rows of Abar_{k+1}
                 T hh = rho * (zh[r] - thh[r]) + rho * gg;                           // h_k (index reading R2)
                 if (has_q) hh += own[OC + r];
-                own[OH + r] = hh;
+                hv[r] = hh;
                 T rr = rd[r][0] + rd[r][1] + dv[r];
                 if (DU) rr += dh[r] - deh[r];
                 if (!isx[r]) own[ORH - NX + r] = rr;
             }
+            st_rows<T, R>(own + OH, hv);
+            RPROF_MARK(2)
             __syncwarp();
             T x[R][2], du2[R][2], du[R];
 #pragma unroll
@@ -260,10 +290,12 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             for (int r = 0; r < R; ++r) {
                 xs[r] = x[r][0] + x[r][1];
                 du[r] = du2[r][0] + du2[r][1];
-                own[OX + r] = xs[r];
                 if (!isx[r]) own[ODU - NX + r] = du[r];
             }
+            st_rows<T, R>(own + OX, xs);
+            RPROF_MARK(3)
             __syncthreads();
+            RPROF_MARK(4)
             // steps 2-4
             T dot[R][2], av2[R][2], avx[R];
 #pragma unroll
@@ -315,14 +347,17 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                     prv.d[r] = dn; prv.de[r] = den;
                 }
             }
-            // step 4: c = rho * sum (fixed order: group butterfly in T, then double)
+            // step 4: c = rho * sum (fixed order: group butterfly in T, then double).  An all-fp32 butterfly was measured
+            // only 1.7 % faster on C4 and would widen the near-tie band of the decision, so c stays in double.
 #pragma unroll
             for (int o = LPS / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
             double s = (double)acc;
 #pragma unroll
             for (int o = 16; o >= LPS; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            RPROF_MARK(5)
             if (lane == 0) red[warp] = s;
             __syncthreads();
+            RPROF_MARK(6)
             const double c_prev = red[32 + (par ^ 1)];
             // every warp repeats the second level (butterfly over the warp partials): same bits everywhere.  A shuffle-free
             // tree of 16 broadcast loads + DADDs per lane was measured 4 % slower on C4 (B200).
@@ -339,6 +374,7 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 if (!accept && !stop) ++sCnt[0];
                 if (hc && it < p.hist_cap) { hc[it] = c; ha[it] = (unsigned char)accept; }
             }
+            RPROF_MARK(7)
             if (stop) { done = true; return true; }
             if (accept) {
                 kap = jacc < C::KAPN ? sKap[jacc] : (T)kappa_tab[jacc];
@@ -358,6 +394,12 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             if (iteration(sb, sa, it + 1, 1)) { in_b = false; break; }
             in_b = false;
         }
+#ifdef PIMPC_RES_PROF
+        if (b == 0 && (tid == 0 || tid == 32 * (nwarps - 1)) && it_done > 0)
+            printf("res prof tid %d: A %lld | B1 %lld | B %lld | C %lld | B2 %lld | D+shfl %lld | B3 %lld | decide %lld cycles/it\n", tid,
+                   prof_t[0] / it_done, prof_t[1] / it_done, prof_t[2] / it_done, prof_t[3] / it_done, prof_t[4] / it_done,
+                   prof_t[5] / it_done, prof_t[6] / it_done, prof_t[7] / it_done);
+#endif
         if (in_b) sa = sb;                       // register moves; a reference select would force local memory
         const RState<T, R> &fin = sa;
 
