@@ -95,6 +95,19 @@ int dalloc(pimpc_s *h, void **p, size_t bytes)
     return PIMPC_OK;
 }
 
+// Device staging area of at least `bytes` (kept in the handle: no cudaMalloc / cudaFree, which synchronise the
+// whole device, on the result path).
+int staging(pimpc_s *h, size_t bytes, void **out)
+{
+    if (h->stage_bytes < bytes) {
+        if (h->stage_buf) { cudaStreamSynchronize(h->stream); cudaFree(h->stage_buf); h->device_bytes -= h->stage_bytes; h->stage_buf = nullptr; h->stage_bytes = 0; }
+        if (cudaMalloc(&h->stage_buf, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, PIMPC_ENOMEM, "cudaMalloc (staging) failed"); }
+        h->stage_bytes = bytes; h->device_bytes += bytes;
+    }
+    *out = h->stage_buf;
+    return PIMPC_OK;
+}
+
 int rec_len(int nb, int nu) { return ((5 * nb + 2 * nu + 3) / 4) * 4; }
 
 struct Sizes {
@@ -239,7 +252,7 @@ int pimpc_destroy(pimpc_t h)
     if (!h->poisoned) cudaStreamSynchronize(h->stream);
     void *ptrs[] = {h->A, h->B, h->e, h->x0, h->uprev, h->Q, h->R, h->P, h->Wdu, h->qbar, h->lo, h->hi, h->dlo, h->dhi,
                     h->H, h->M, h->S, h->X, h->DU, h->ctl, h->partial, h->hist_c, h->hist_a, h->err,
-                    h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab, h->spartial, h->coop_buf};
+                    h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab, h->spartial, h->coop_buf, h->stage_buf};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (auto &e : h->ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();
@@ -418,28 +431,24 @@ int pimpc_get(pimpc_t h, void *x, void *u, void *du, pimpc_result *res)
     // gather into device staging when the destination is host memory
     void *dx = nullptr, *du_ = nullptr, *ddu = nullptr;
     pimpc_result *dres = nullptr;
-    std::vector<void *> tmp;
-    auto stage = [&](void *user, size_t bytes, void **dev) -> int {
-        if (!user) { *dev = nullptr; return PIMPC_OK; }
-        if (is_device_ptr(user)) { *dev = user; return PIMPC_OK; }
-        cudaError_t e = cudaMalloc(dev, bytes);
-        if (e != cudaSuccess) { cudaGetLastError(); return fail(h, PIMPC_ENOMEM, "cudaMalloc (staging) failed"); }
-        tmp.push_back(*dev);
-        return PIMPC_OK;
-    };
-    rc = stage(x, nst * h->nx * esz, &dx);
-    if (!rc) rc = stage(u, nst * h->nu * esz, &du_);
-    if (!rc) rc = stage(du, nst * h->nu * esz, &ddu);
-    if (!rc) rc = stage(res, (size_t)h->batch * sizeof(pimpc_result), (void **)&dres);
+    const size_t bx = nst * h->nx * esz, bu = nst * h->nu * esz, br = (size_t)h->batch * sizeof(pimpc_result);
+    auto al = [](size_t v) { return (v + 255) / 256 * 256; };
+    const bool hx = x && !is_device_ptr(x), hu = u && !is_device_ptr(u), hd = du && !is_device_ptr(du), hr = res && !is_device_ptr(res);
+    const size_t need = (hx ? al(bx) : 0) + (hu ? al(bu) : 0) + (hd ? al(bu) : 0) + (hr ? al(br) : 0);
+    unsigned char *sb = nullptr;
+    if (need) { rc = staging(h, need, (void **)&sb); if (rc) return rc; }
+    size_t off = 0;
+    dx = hx ? sb + off : x; off += hx ? al(bx) : 0;
+    du_ = hu ? sb + off : u; off += hu ? al(bu) : 0;
+    ddu = hd ? sb + off : du; off += hd ? al(bu) : 0;
+    dres = hr ? (pimpc_result *)(sb + off) : res;
     if (!rc) rc = launch_gather(h, dx, du_, ddu, dres) < 0 ? PIMPC_ECUDA : PIMPC_OK;
     if (!rc && x && dx != x) rc = copy_out(h, x, dx, nst * h->nx * esz);
     if (!rc && u && du_ != u) rc = copy_out(h, u, du_, nst * h->nu * esz);
     if (!rc && du && ddu != du) rc = copy_out(h, du, ddu, nst * h->nu * esz);
     if (!rc && res && (void *)dres != (void *)res) rc = copy_out(h, res, dres, (size_t)h->batch * sizeof(pimpc_result));
     h->info.total_launches += 1;
-    int rc2 = rc ? rc : deferred_error(h);     // synchronises
-    for (void *p : tmp) cudaFree(p);
-    return rc2;
+    return rc ? rc : deferred_error(h);        // synchronises
 }
 
 static int state_width(pimpc_s *h, int which)
@@ -460,11 +469,10 @@ int pimpc_get_state(pimpc_t h, int which, void *out)
     const size_t bytes = (size_t)h->batch * h->N * w * h->esz;
     void *dev = out;
     const bool host = !is_device_ptr(out);
-    if (host) { if (cudaMalloc(&dev, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, PIMPC_ENOMEM, "cudaMalloc (staging) failed"); } }
+    if (host) { rc = staging(h, bytes, &dev); if (rc) return rc; }
     rc = launch_state_io(h, which, dev, 0) < 0 ? PIMPC_ECUDA : PIMPC_OK;
     if (!rc && host) rc = copy_out(h, out, dev, bytes);
     if (!rc) { cudaError_t e = cudaStreamSynchronize(h->stream); if (e != cudaSuccess) { h->poisoned = 1; rc = fail(h, PIMPC_ECUDA, cudaGetErrorString(e)); } }
-    if (host) cudaFree(dev);
     return rc;
 }
 
@@ -478,11 +486,11 @@ int pimpc_set_state(pimpc_t h, int which, const void *in)
     void *dev = const_cast<void *>(in);
     const bool host = !is_device_ptr(in);
     if (host) {
-        if (cudaMalloc(&dev, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, PIMPC_ENOMEM, "cudaMalloc (staging) failed"); }
+        rc = staging(h, bytes, &dev); if (rc) return rc;
         rc = copy_in(h, dev, in, bytes);
     }
     if (!rc) rc = launch_state_io(h, which, dev, 1) < 0 ? PIMPC_ECUDA : PIMPC_OK;
-    if (host) { cudaStreamSynchronize(h->stream); cudaFree(dev); }
+    if (host) cudaStreamSynchronize(h->stream);
     return rc;
 }
 

@@ -93,6 +93,8 @@ struct pimpc_s {
     double *spartial = nullptr;              // [2][grid][MAXI] partial sums of c of the STREAM engine
     size_t spartial_cap = 0;
     bool blob_dirty = true;
+    void *stage_buf = nullptr;               // device staging of results bound for host memory (grown on demand, kept)
+    size_t stage_bytes = 0;
     void *coop_buf = nullptr;                // tagged exchange words of the COOP engine (partials of c, boundary iterates)
     size_t coop_bytes = 0;
 
