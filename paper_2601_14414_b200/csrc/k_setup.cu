@@ -113,21 +113,33 @@ __device__ __forceinline__ bool gj_rows(double (&S)[W], double *rowb, const int 
     for (int p = 0; p < NPIV; ++p) {
         __syncwarp();
         if (li == p) {
+            if constexpr (W % 2 == 0) {                        // 16-byte stores / broadcast loads of the pivot row
 #pragma unroll
-            for (int j = 0; j < W; ++j) rowb[j] = S[j];
+                for (int j = 0; j < W; j += 2) *reinterpret_cast<double2 *>(rowb + j) = make_double2(S[j], S[j + 1]);
+            } else {
+#pragma unroll
+                for (int j = 0; j < W; ++j) rowb[j] = S[j];
+            }
         }
         __syncwarp();
         const double piv = rowb[p], colv = S[p];
         if (!(piv > 0.0) || !isfinite(piv)) ok = false;
         const double inv = 1.0 / piv;
+        // one exchange step as a rank-1 update S[i][:] -= f_i * pivot_row with f_i = S[i][p] / piv for i != p and
+        // f_p = 1 - 1/piv (so that the pivot row becomes pivot_row / piv); column p is then overwritten with -f_i
+        // (1/piv in the pivot row).  One select per step instead of one per element.
+        const double f = (li == p) ? 1.0 - inv : colv * inv;
+        if constexpr (W % 2 == 0) {
 #pragma unroll
-        for (int j = 0; j < W; ++j) {
-            const double r = rowb[j];
-            double v;
-            if (li == p) v = (j == p) ? inv : r * inv;
-            else v = (j == p) ? -colv * inv : S[j] - colv * r * inv;
-            S[j] = v;
+            for (int j = 0; j < W; j += 2) {
+                const double2 r2 = *reinterpret_cast<const double2 *>(rowb + j);
+                S[j] = fma(-f, r2.x, S[j]); S[j + 1] = fma(-f, r2.y, S[j + 1]);
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < W; ++j) S[j] = fma(-f, rowb[j], S[j]);
         }
+        S[p] = (li == p) ? inv : -f;
     }
     __syncwarp();
     return ok;
@@ -138,7 +150,8 @@ __global__ void __launch_bounds__(128) k_setup_small(Prob<T> p)
 {
     constexpr int NB = NX + NU, LPS = pow2ceil_k(NB), SPW = 32 / LPS, GPB = 4 * SPW, TS = LPS + 1;
     constexpr int GSZ = (NX * LPS > LPS * TS ? NX * LPS : LPS * TS) + LPS;
-    __shared__ double sm[GPB * GSZ];
+    static_assert(GSZ % 2 == 0 && LPS % 2 == 0, "16-byte alignment of the per-group buffers");
+    __shared__ __align__(16) double sm[GPB * GSZ];
     const int tid = threadIdx.x, g = tid / LPS, li = tid % LPS, N = p.N;
     const long long nst = (long long)p.batch * N, sraw = (long long)blockIdx.x * GPB + g;
     const bool act = sraw < nst;
@@ -163,29 +176,29 @@ __global__ void __launch_bounds__(128) k_setup_small(Prob<T> p)
     }
     __syncwarp();
     double S[LPS];
-    {
-        double acc[LPS];
+    const double rl = last ? 0.0 : rho;                        // the terminal stage has no Abar_{k+1} term
 #pragma unroll
-        for (int j = 0; j < LPS; ++j) acc[j] = (j == li && li >= NX) ? 1.0 : 0.0;      // the [0 I] rows of Abar
+    for (int j = 0; j < LPS; ++j) {
+        double s = 0.0;
+        if (rowok && j < NB) {
+            if (li < NX && j < NX) s = (double)Qx[li * NX + j];
+            else if (li >= NX && j >= NX) s = (double)Rx[(li - NX) * NU + (j - NX)];
+            if (j == li) s += rho + (li >= NX ? rl : 0.0);      // rho I and the [0 I] rows of rho Abar^T Abar
+        } else if (j == li) s = 1.0;                            // pad rows: identity
+        S[j] = s;
+    }
 #pragma unroll
-        for (int r = 0; r < NX; ++r) {
-            const double ai = buf[r * LPS + li];
+    for (int r = 0; r < NX; ++r) {                              // + rho [A B]^T [A B], accumulated in place
+        const double ai = rl * buf[r * LPS + li];
 #pragma unroll
-            for (int j = 0; j < LPS; ++j) acc[j] += ai * buf[r * LPS + j];
-        }
-#pragma unroll
-        for (int j = 0; j < LPS; ++j) {
-            double s = 0.0;
-            if (rowok && j < NB) {
-                if (li < NX && j < NX) s = (double)Qx[li * NX + j];
-                else if (li >= NX && j >= NX) s = (double)Rx[(li - NX) * NU + (j - NX)];
-                if (j == li) s += rho;
-                if (!last) s += rho * acc[j];
-            } else if (j == li) s = 1.0;                        // pad rows: identity
-            if (!isfinite(s)) finite = false;
-            S[j] = s;
+        for (int j = 0; j < LPS; j += 2) {
+            const double2 v = *reinterpret_cast<const double2 *>(buf + r * LPS + j);
+            S[j] = fma(ai, v.x, S[j]); S[j + 1] = fma(ai, v.y, S[j + 1]);
         }
     }
+#pragma unroll
+    for (int j = 0; j < LPS; ++j)
+        if (!isfinite(S[j])) finite = false;
     bool ok = gj_rows<LPS, NB>(S, rowb, li);
 #pragma unroll
     for (int j = 0; j < LPS; ++j) buf[li * TS + j] = S[j];
