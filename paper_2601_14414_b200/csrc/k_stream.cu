@@ -100,6 +100,16 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 template <typename T> __device__ __forceinline__ T clips(T v, T lo, T hi) { return fmin(fmax(v, lo), hi); }
+__device__ __forceinline__ void ld4s(const float *p, float (&o)[4])
+{
+    const float4 v = *reinterpret_cast<const float4 *>(p);
+    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void ld4s(const double *p, double (&o)[4])
+{
+    const double2 a = *reinterpret_cast<const double2 *>(p), b = *reinterpret_cast<const double2 *>(p + 2);
+    o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
+}
 
 // ---- pack: blob'_j of every (instance, j = -1..N-1), once per solve after the cache kernel ----------
 template <typename T, int NX, int NU>
@@ -290,10 +300,27 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                 if (has_next && ci < NB) {
                     const int r0 = prt * RP, r1 = r0 + RP < NX ? r0 + RP : NX;
                     T a0 = (T)0, a1 = (T)0;
-                    for (int r = r0; r < r1; ++r) {
-                        const T a = AB[r * NB + ci];
-                        a0 += a * wv[r];
-                        if (ci >= NX) a1 += a * dv[r];
+                    if constexpr (NX % NPART == 0 && RP % 4 == 0) {        // compile-time trip count, 16-byte vector loads
+                        const T *ABp = AB + r0 * NB + ci;
+                        const bool ucol = ci >= NX;
+#pragma unroll
+                        for (int rr = 0; rr < RP; rr += 4) {
+                            T w4[4], d4[4];
+                            ld4s(wv + r0 + rr, w4);
+                            ld4s(dv + r0 + rr, d4);
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) {
+                                const T a = ABp[(rr + q) * NB];
+                                a0 += a * w4[q];
+                                if (ucol) a1 += a * d4[q];
+                            }
+                        }
+                    } else {
+                        for (int r = r0; r < r1; ++r) {
+                            const T a = AB[r * NB + ci];
+                            a0 += a * wv[r];
+                            if (ci >= NX) a1 += a * dv[r];
+                        }
                     }
                     gp[prt * IP + ci] = a0;
                     if (ci >= NX) rp[prt * IP + ci - NX] = a1;
@@ -325,12 +352,19 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                 // ---- D: xbar_{j+1} = H_j h_j, H stored once: C[s][i] = H[i][(i+s) % NB] ----
                 if (ci < NB && !first) {
                     T a0 = (T)0, a1 = (T)0;
-                    for (int s = prt; s < C::NS; s += NPART) {
-                        const T *Cs = Cb + s * NB;
-                        a0 += Cs[ci] * hv[ci + s];
-                        if (s > 0 && 2 * s != NB) {
-                            int im = ci - s; if (im < 0) im += NB;
-                            a1 += Cs[im] * hv[im];
+                    constexpr int QD = (C::NS + NPART - 1) / NPART;
+                    const T *Cp = Cb + prt * NB, *hp = hv + ci + prt;
+                    const int im0 = ci - prt;
+#pragma unroll
+                    for (int q = 0; q < QD; ++q) {                         // s = prt + q NPART: same order as a rolled loop
+                        const int s = prt + q * NPART;
+                        if (s < C::NS) {
+                            const T *Cs = Cp + q * NPART * NB;
+                            a0 += Cs[ci] * hp[q * NPART];
+                            if (s > 0 && 2 * s != NB) {
+                                const int imw = im0 - q * NPART;           // (ci - s); h is stored twice, so hv[imw + NB] = h[(ci - s) mod NB]
+                                a1 += Cs[imw < 0 ? imw + NB : imw] * hv[imw + NB];
+                            }
                         }
                     }
                     xp[prt * IP + ci] = a0 + a1;
