@@ -202,6 +202,38 @@ def us_per_iteration(torch, pimpc, prob, dtype, iters, reps=7, engine="auto"):
             "engine": info["engine"], "grid": info["grid"], "block": info["block"]}
 
 
+def cstr_closed_loop(torch, pimpc, N=5000, K=1000, steps=6):
+    """receding-horizon stepping at the paper's CSTR scale (N = 5000, 1000
+    iterations per MPC step; its GPU code: 0.526 s median per step on an RTX 3080).  Per step: linearise on the host,
+    upload the stage data, a0, shift warm start, K iterations, read u_0; the plant advances with u_0."""
+    out = {}
+    for dt in ("f64", "f32"):
+        x = np.array(wl.CSTR["x_init"]); u = np.array([wl.CSTR["u_init"]]); t = 0.0
+        s = pimpc.Solver(4, 2, N, 1, dtype=dt)
+        ms, ca = [], []
+        for step in range(steps):
+            pp = wl.pad_problem(wl.cstr_problem(x, u, t, N, iters=K), 4, 2)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            s.set_problem(pp)
+            if step:
+                s.shift(1)
+            s.solve(K)
+            _, ug, _, _ = s.get()
+            ms.append(1e3 * (time.perf_counter() - t0))
+            u = ug[0, 0, :1].astype(np.float64)
+            x = wl.cstr_plant_step(x, u, t); t += wl.CSTR["Ts"]
+            ca.append(float(x[0]))
+        info = s.get_info()
+        s.close()
+        out[dt] = {"ms_per_mpc_step_median": statistics.median(ms[1:]), "ms_per_mpc_step_max": max(ms[1:]),
+                   "iter_kernel_ms": info["iter_ms"], "cache_kernel_ms": info["setup_ms"], "engine": info["engine"],
+                   "grid": info["grid"], "C_A_after_steps": ca[-1]}
+    out["config"] = {"N": N, "iters_per_step": K, "steps_timed": steps - 1, "shape": "(2,1) embedded in (4,2)",
+                     "paper_gpu_s_per_step": 0.526}
+    return out
+
+
 def extras(torch, pimpc, pk):
     out = {}
     out["C1_f64"] = us_per_iteration(torch, pimpc, wl.config1(), "f64", 500)
@@ -212,6 +244,7 @@ def extras(torch, pimpc, pk):
         sweep[str(N)] = us_per_iteration(torch, pimpc, wl.config3(N), "f32", 1000, reps=5)
     out["C3_f32_us_per_iter_vs_N"] = sweep
     out["C3_flatness_t10000_over_t10"] = sweep["10000"]["us_per_iter"] / max(sweep["10"]["us_per_iter"], 1e-9)
+    out["CSTR_closed_loop"] = cstr_closed_loop(torch, pimpc)
     p5 = wl.config5()
     for dt, esz in (("f32", 4), ("f64", 8)):
         s = pimpc.Solver(p5.nx, p5.nu, p5.N, p5.batch, dtype=dt, rho=p5.rho)

@@ -157,6 +157,13 @@ int pimpc_get_cache(pimpc_t h, void *M, void *H);
 /* Cold start: all iterates = 0 (R9). */
 int pimpc_reset(pimpc_t h);
 
+/* Receding-horizon warm start (Alg. 1 takes its initial iterates "such as from warm-start" and returns them for the
+ * next MPC step; reading R18): the current iterate of every instance is shifted by `steps` stages,
+ * stage k takes the values of stage k + steps (Z, V, TH, BE, LA, D, DE); the last `steps` stages repeat the old last
+ * stage.  0 <= steps < N, else EINVAL.  Asynchronous on the handle's stream.  X and DU (outputs of the last
+ * iteration) are not touched. */
+int pimpc_shift(pimpc_t h, int steps);
+
 /* Wait for the handle's stream; returns a deferred device-side error if one was raised. */
 int pimpc_sync(pimpc_t h);
 

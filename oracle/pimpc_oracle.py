@@ -134,3 +134,18 @@ def cache(A, B, Q, R, *, P=None, Wdu=None, has_du=False, rho=1.0):
     if rc != 0:
         raise RuntimeError(f"pimpc_oracle_cache failed: {rc}")
     return M, H
+
+
+def shift_warm(warm, steps=1):
+    """Receding-horizon warm start (reading R18): stage k takes the iterate of stage
+    k + steps, the last `steps` stages repeat the old last stage.  `warm` = dict of [N, w] arrays."""
+    out = {}
+    for name, a in warm.items():
+        if a is None:
+            out[name] = None
+            continue
+        a = np.asarray(a, dtype=np.float64)
+        N = a.shape[0]
+        idx = np.minimum(np.arange(N) + steps, N - 1)
+        out[name] = a[idx].copy()
+    return out

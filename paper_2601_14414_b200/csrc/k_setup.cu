@@ -314,6 +314,30 @@ __global__ void k_state_io(Prob<T> p, int which, T *buf, int set)
     }
 }
 
+// Warm-start shift (reading R18): record k of the next rotating buffer = record min(k + steps, N-1) of the current one.
+template <typename T>
+__global__ void k_shift(Prob<T> p, int steps)
+{
+    const int b = blockIdx.y;
+    const InstCtl c = p.ctl[b];
+    const int dst = (c.i_cur + 1) % 3;
+    const T *src = p.S + (size_t)c.i_cur * p.buf_stride;
+    T *out = p.S + (size_t)dst * p.buf_stride;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < p.N * p.rec; idx += gridDim.x * blockDim.x) {
+        const int k = idx / p.rec, i = idx - k * p.rec;
+        const int ks = k + steps < p.N ? k + steps : p.N - 1;
+        out[p.st(b, k) + i] = src[p.st(b, ks) + i];
+    }
+}
+
+// after k_shift: the shifted buffer becomes the current iterate
+__global__ void k_advance_cur(InstCtl *ctl, int batch)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    ctl[b].i_cur = (ctl[b].i_cur + 1) % 3;
+}
+
 __global__ void k_zero_ctl(InstCtl *ctl, int batch, double c0)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
@@ -415,6 +439,18 @@ int launch_state_io(pimpc_s *h, int which, void *buf, int set)
         k_state_io<float><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<float>(h, 0.0), which, (float *)buf, set);
     PIMPC_CUDA_TRY(h, cudaGetLastError());
     return 1;
+}
+
+int launch_shift(pimpc_s *h, int steps)
+{
+    const int work = h->N * h->rec;
+    const int th = 256, bl = min(64, (work + th - 1) / th);
+    if (h->dtype == PIMPC_F64) k_shift<double><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<double>(h, 0.0), steps);
+    else k_shift<float><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<float>(h, 0.0), steps);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    k_advance_cur<<<(h->batch + 127) / 128, 128, 0, h->stream>>>(h->ctl, h->batch);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 2;
 }
 
 int launch_zero_state(pimpc_s *h)

@@ -523,6 +523,18 @@ int pimpc_reset(pimpc_t h)
     return launch_zero_state(h) < 0 ? PIMPC_ECUDA : PIMPC_OK;
 }
 
+int pimpc_shift(pimpc_t h, int steps)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    if (steps < 0 || steps >= h->N) return fail(h, PIMPC_EINVAL, "shift: steps must be in [0, N)");
+    if (steps == 0) return PIMPC_OK;
+    const int n = launch_shift(h, steps);
+    if (n < 0) return PIMPC_ECUDA;
+    h->info.total_launches += n;
+    return PIMPC_OK;
+}
+
 int pimpc_sync(pimpc_t h)
 {
     int rc = check_handle(h);

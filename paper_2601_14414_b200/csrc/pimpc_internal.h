@@ -124,6 +124,7 @@ bool stream_supported(const pimpc_s *h, std::string *why);
 int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res_dev);
 int launch_state_io(pimpc_s *h, int which, void *buf_dev, int set);
 int launch_zero_state(pimpc_s *h);
+int launch_shift(pimpc_s *h, int steps);              // warm-start shift of the current iterate (reading R18)
 
 #define PIMPC_CUDA_TRY(h, expr)                                                         \
     do {                                                                                \

@@ -69,6 +69,7 @@ SYMBOLS = {
     "pimpc_get_history": (_i, [_vp, _vp, _vp]),
     "pimpc_get_cache": (_i, [_vp, _vp, _vp]),
     "pimpc_reset": (_i, [_vp]),
+    "pimpc_shift": (_i, [_vp, _i]),
     "pimpc_sync": (_i, [_vp]),
     "pimpc_get_info": (_i, [_vp, ctypes.POINTER(pimpc_info)]),
     "pimpc_last_error": (ctypes.c_char_p, [_vp]),
@@ -206,6 +207,9 @@ class Solver:
 
     def reset(self):
         self._ck(self.lib.pimpc_reset(self.h))
+
+    def shift(self, steps=1):
+        self._ck(self.lib.pimpc_shift(self.h, int(steps)))
 
     def get(self, x=None, u=None, du=None, res=None):
         """Fill caller-provided buffers (numpy or torch); returns (x, u, du, res) with numpy defaults."""

@@ -228,3 +228,85 @@ def random_ltv(nx: int, nu: int, N: int, batch: int = 1, *, seed: int = 0, affin
         kw = dict(du_lo=-du_bound * np.ones(nu), du_hi=du_bound * np.ones(nu))
     return Problem(f"rand-{nx}-{nu}-{N}", nx, nu, N, batch, A, B, Q, R, lo, hi, x0, e=e, P=P, Wdu=W, qbar=qb,
                    u_prev=up, rho=1.0, iters=200, **kw)
+
+
+# --------------------------------------------------------------------------------------------
+# CSTR with online linearisation: closed-loop / RTI stepping workload
+# --------------------------------------------------------------------------------------------
+CSTR = dict(CAi=10.0, k0=34930800.0, EaR=5963.6, Ts=0.5, x_init=(8.57, 311.27), u_init=300.0, ref=2.0,
+            lo=(0.0, 250.0, 250.0), hi=(12.0, 450.0, 350.0), Wy=1.0, Wu=0.0, Wdu=0.1)
+
+
+def cstr_f(x, u, t):
+    """dC_A/dt, dT/dt of the CSTR as printed at PAPER.md:399; inlet disturbance T_i = 298.15 + 5 sin(0.05 t)."""
+    ca, T = float(x[0]), float(x[1])
+    r = CSTR["k0"] * np.exp(-CSTR["EaR"] / T) * ca
+    Ti = 298.15 + 5.0 * np.sin(0.05 * t)
+    return np.array([CSTR["CAi"] - ca - r, Ti + 0.3 * float(u[0]) - 1.3 * T + 11.92 * r])
+
+
+def cstr_plant_step(x, u, t):
+    """The plant, advanced by one sampling period with the paper's forward-Euler discretisation (T_s = 0.5 min)."""
+    return np.asarray(x, np.float64) + CSTR["Ts"] * cstr_f(x, u, t)
+
+
+def cstr_problem(x, u_prev, t0, N, *, rho=1.0, iters=1000, ref=None) -> Problem:
+    """One MPC step: the model linearised around the current state and the previous input,
+    x_{k+1} = A x_k + B u_k + e_k with the disturbance sampled along the horizon in e_k; output y = C_A tracked
+    to `ref` (W_y = 1, W_u = 0, W_du = 0.1).  The reference value and the boxes are this build's choice (the paper
+    shows them only in a figure); DESIGN.md "Input recipe"."""
+    Ts, k0, EaR = CSTR["Ts"], CSTR["k0"], CSTR["EaR"]
+    x = np.asarray(x, np.float64); u = np.asarray(u_prev, np.float64).reshape(1)
+    ca, T = x
+    kk = k0 * np.exp(-EaR / T)
+    dk = kk * EaR / (T * T)                                  # d/dT of k0 exp(-EaR/T)
+    J = np.array([[-1.0 - kk, -dk * ca], [11.92 * kk, -1.3 + 11.92 * dk * ca]])
+    A = np.eye(2) + Ts * J
+    B = np.array([[0.0], [Ts * 0.3]])
+    e0 = x + Ts * cstr_f(x, u, t0) - A @ x - B @ u            # affine term of the linearisation at (x, u, t0)
+    tk = t0 + Ts * np.arange(N)                               # the disturbance T_i(t) enters dT/dt additively
+    e = np.tile(e0, (N, 1))
+    e[:, 1] += Ts * 5.0 * (np.sin(0.05 * tk) - np.sin(0.05 * t0))
+    r = CSTR["ref"] if ref is None else ref
+    Q = np.diag([CSTR["Wy"], 0.0]); R = np.array([[CSTR["Wu"]]])
+    qbar = np.array([CSTR["Wy"] * r, 0.0, 0.0])
+    return Problem("CSTR", 2, 1, N, 1, np.tile(A, (1, N, 1, 1)), np.tile(B, (1, N, 1, 1)), Q, R,
+                   np.array(CSTR["lo"]), np.array(CSTR["hi"]), x[None, :].copy(), e=e[None], Wdu=np.array([[CSTR["Wdu"]]]),
+                   qbar=qbar, u_prev=u[None, :].copy(), rho=rho, iters=iters, tol=0.0, dtypes=("f64", "f32"),
+                   meta=dict(t0=t0))
+
+
+def pad_problem(p: Problem, nx2: int, nu2: int) -> Problem:
+    """Embed p in a larger shape by adding decoupled zero states / inputs (A, B blocks 0, unit weights, boxes
+    [-1, 1], zero initial state): the added components stay exactly 0 in every iterate and add exactly 0 to the
+    residual, so the original components are unchanged.  Lets a shape without a fused-engine instantiation
+    (the CSTR's nx = 2, nu = 1) run on one that has (4, 2).  Pure data marshalling."""
+    nx, nu, N, b = p.nx, p.nu, p.N, p.batch
+    assert nx2 >= nx and nu2 >= nu
+    A = np.zeros((b, N, nx2, nx2)); A[:, :, :nx, :nx] = p.A
+    B = np.zeros((b, N, nx2, nu2)); B[:, :, :nx, :nu] = p.B
+
+    def blk(M, n, n2, fill):
+        if M is None:
+            return None
+        out = np.eye(n2) * fill
+        out[:n, :n] = M
+        return out
+
+    def vec(xpart, upart, fx, fu):
+        return np.concatenate([xpart, np.full(nx2 - nx, fx), upart, np.full(nu2 - nu, fu)])
+
+    e = None
+    if p.e is not None:
+        e = np.zeros((b, N, nx2)); e[:, :, :nx] = p.e
+    x0 = np.zeros((b, nx2)); x0[:, :nx] = p.x0
+    up = None
+    if p.u_prev is not None:
+        up = np.zeros((b, nu2)); up[:, :nu] = p.u_prev
+    qbar = None if p.qbar is None else vec(p.qbar[:nx], p.qbar[nx:], 0.0, 0.0)
+    pad_u = lambda v, f: None if v is None else np.concatenate([v, np.full(nu2 - nu, f)])
+    return Problem(p.name + "-pad", nx2, nu2, N, b, A, B, blk(p.Q, nx, nx2, 1.0), blk(p.R, nu, nu2, 1.0),
+                   vec(p.lo[:nx], p.lo[nx:], -1.0, -1.0), vec(p.hi[:nx], p.hi[nx:], 1.0, 1.0), x0, e=e,
+                   P=blk(p.P, nx, nx2, 1.0), Wdu=blk(p.Wdu, nu, nu2, 0.0), qbar=qbar,
+                   du_lo=pad_u(p.du_lo, -1.0), du_hi=pad_u(p.du_hi, 1.0), u_prev=up, rho=p.rho, iters=p.iters,
+                   tol=p.tol, dtypes=p.dtypes, meta=dict(p.meta, pad_of=(nx, nu)))

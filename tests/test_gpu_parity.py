@@ -227,6 +227,56 @@ def test_coop_engine_unbounded_plain_admm_early_stop_warm_start(oracle, pimpc, c
     assert parity.relerr(s.get_state("Z")[0], o.Z) <= 1e-9
 
 
+# ---- NEXT row f1: receding-horizon stepping with shift warm start ----------------
+@pytest.mark.parametrize("engine", ["auto", "coop", "stream", "staged"])
+def test_closed_loop_cstr_shift_warm_start(oracle, pimpc, engine):
+    """Four MPC steps of the online-linearised CSTR: per step new stage data (set_stages + a0), pimpc_shift(1) of the
+    previous iterates, K iterations; the plant advances with the oracle's u_0.  The CUDA path runs the (2, 1)
+    problem embedded in the (4, 2) shape (workloads.pad_problem), the oracle the original one."""
+    N, K, T = 60, 120, 4
+    x = np.array(wl.CSTR["x_init"]); u = np.array([wl.CSTR["u_init"]]); t = 0.0
+    s = pimpc.Solver(4, 2, N, 1, dtype="f64", engine=engine, history=K)
+    real = [0, 1, 4]
+    warm = None
+    for step in range(T):
+        p = wl.cstr_problem(x, u, t, N, iters=K)
+        s.set_problem(wl.pad_problem(p, 4, 2))
+        if step:
+            s.shift(1)
+        s.solve(K)
+        o = oracle.solve(**p.instance(0), max_iters=K, tol=0.0, warm=None if warm is None else oracle.shift_warm(warm, 1))
+        c, acc = s.get_history()
+        assert list(acc[0]) == list(o.acc_hist)
+        np.testing.assert_allclose(c[0], o.c_hist, rtol=1e-7)
+        for name in ("Z", "V", "TH", "BE", "LA", "X"):
+            g = s.get_state(name)[0]
+            assert parity.relerr(g[:, real], getattr(o, name)) <= 1e-9, (step, name)
+            assert float(np.max(np.abs(np.delete(g, real, axis=1)))) == 0.0          # the embedding stays exactly zero
+        xg, ug, dug, res = s.get()
+        assert parity.relerr(ug[0, :, :1], o.u) <= 1e-9 and parity.relerr(dug[0, :, :1], o.DU) <= 1e-9
+        warm = dict(Z=o.Z, V=o.V, TH=o.TH, BE=o.BE, LA=o.LA)
+        u = o.u[0].copy()
+        x = wl.cstr_plant_step(x, u, t); t += wl.CSTR["Ts"]
+    assert x[0] < wl.CSTR["x_init"][0]                    # the loop moves C_A towards the reference
+
+
+def test_shift_argument_validation_and_identity(pimpc):
+    p = wl.quadrotor_ltv(12, 2, iters=30, tol=0.0)
+    s = pimpc.Solver(p.nx, p.nu, p.N, p.batch, dtype="f32"); s.set_problem(p); s.solve(30)
+    z = s.get_state("Z"); th = s.get_state("TH"); d = s.get_state("D")
+    s.shift(0)
+    np.testing.assert_array_equal(s.get_state("Z"), z)
+    s.shift(3)
+    idx = np.minimum(np.arange(p.N) + 3, p.N - 1)
+    np.testing.assert_array_equal(s.get_state("Z"), z[:, idx])
+    np.testing.assert_array_equal(s.get_state("TH"), th[:, idx])
+    np.testing.assert_array_equal(s.get_state("D"), d[:, idx])
+    for bad in (-1, p.N):
+        with pytest.raises(pimpc.PimpcError) as e:
+            s.shift(bad)
+        assert e.value.code == pimpc.EINVAL
+
+
 # ---- odd shapes, optional terms, edge cases -----------------------------------------------------
 @pytest.mark.parametrize("engine", ENGINES_SMALL)
 @pytest.mark.parametrize("dtype", ["f64", "f32"])

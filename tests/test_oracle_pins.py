@@ -280,3 +280,21 @@ def test_generators_are_deterministic_and_shaped():
     assert c5.A.shape == (2, 7, 48, 48) and c5.nu == 12
     # forward-Euler chain: spectral radius close to 1 (SURVEY.md section 8(d) C5 probe: ~1.005)
     assert 0.99 < np.max(np.abs(np.linalg.eigvals(c5.A[0, 0]))) < 1.02
+
+
+def test_shift_warm_start_definition_and_benefit(oracle):
+    """Reading R18 (receding-horizon warm start): shift_warm is the index map k -> min(k + steps, N-1); on an LTI
+    problem re-solved one step later from the plant's next state, the shifted warm start begins with a far smaller
+    residual than the cold start (why Alg. 1 takes its initial iterates from the previous MPC step)."""
+    a = np.arange(12.0).reshape(6, 2)
+    w = oracle.shift_warm({"Z": a, "D": None}, 2)
+    assert w["D"] is None
+    np.testing.assert_array_equal(w["Z"], a[[2, 3, 4, 5, 5, 5]])
+    p = wl.config1()
+    o = oracle.solve(**p.instance(0), max_iters=3000, tol=0.0)
+    x1 = p.A[0, 0] @ p.x0[0] + p.B[0, 0] @ o.u[0]
+    kw = dict(p.instance(0)); kw["x0"] = x1; kw["u_prev"] = o.u[0]
+    warm = oracle.shift_warm(dict(Z=o.Z, V=o.V, TH=o.TH, BE=o.BE, LA=o.LA), 1)
+    cold = oracle.solve(**kw, max_iters=2, tol=0.0)
+    hot = oracle.solve(**kw, max_iters=2, tol=0.0, warm=warm)
+    assert hot.c_hist[0] < 0.2 * cold.c_hist[0]           # 0.42 vs 4.1 on config 1 (short horizon: the tail is new)
