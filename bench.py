@@ -245,6 +245,13 @@ def extras(torch, pimpc, pk):
     out["C3_f32_us_per_iter_vs_N"] = sweep
     out["C3_flatness_t10000_over_t10"] = sweep["10000"]["us_per_iter"] / max(sweep["10"]["us_per_iter"], 1e-9)
     out["CSTR_closed_loop"] = cstr_closed_loop(torch, pimpc)
+    # the paper's Table I grid (its GPU code: 530-620 us per iteration at every size)
+    t1 = {}
+    for nx, nu in wl.TABLE1_SHAPES:
+        for N in wl.TABLE1_HORIZONS:
+            r = us_per_iteration(torch, pimpc, wl.paper_random(nx, nu, N), "f64", 200, reps=3)
+            t1[f"{nx},{nu},{N}"] = round(r["us_per_iter"], 2)
+    out["paper_table1_us_per_iter_f64"] = t1
     p5 = wl.config5()
     for dt, esz in (("f32", 4), ("f64", 8)):
         s = pimpc.Solver(p5.nx, p5.nu, p5.N, p5.batch, dtype=dt, rho=p5.rho)

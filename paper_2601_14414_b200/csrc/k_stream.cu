@@ -601,7 +601,16 @@ int run_stream_t(pimpc_s *h, int iters, double tol)
     return launches + 1;
 }
 
-bool stream_shape(const pimpc_s *h) { return (h->nx == 48 && h->nu == 12) || (h->nx == 12 && h->nu == 4) || (h->nx == 4 && h->nu == 2); }
+// (nx, nu) with a STREAM instantiation: the three BASELINE.json shapes and the paper's Table I shapes
+#define PIMPC_STREAM_SHAPES(X) X(4, 2) X(12, 4) X(48, 12) X(10, 3) X(20, 6) X(30, 10) X(50, 15)
+
+bool stream_shape(const pimpc_s *h)
+{
+#define X(NX_, NU_) if (h->nx == NX_ && h->nu == NU_) return true;
+    PIMPC_STREAM_SHAPES(X)
+#undef X
+    return false;
+}
 
 } // namespace
 
@@ -618,7 +627,10 @@ int run_stream(pimpc_s *h, int iters, double tol)
 {
     if (!stream_shape(h)) { h->errmsg = "STREAM engine not applicable"; return PIMPC_EINVAL; }
     const bool d = h->dtype == PIMPC_F64;
-    if (h->nx == 48) return d ? run_stream_t<double, 48, 12>(h, iters, tol) : run_stream_t<float, 48, 12>(h, iters, tol);
-    if (h->nx == 12) return d ? run_stream_t<double, 12, 4>(h, iters, tol) : run_stream_t<float, 12, 4>(h, iters, tol);
-    return d ? run_stream_t<double, 4, 2>(h, iters, tol) : run_stream_t<float, 4, 2>(h, iters, tol);
+#define X(NX_, NU_) \
+    if (h->nx == NX_ && h->nu == NU_) return d ? run_stream_t<double, NX_, NU_>(h, iters, tol) : run_stream_t<float, NX_, NU_>(h, iters, tol);
+    PIMPC_STREAM_SHAPES(X)
+#undef X
+    h->errmsg = "STREAM engine not applicable";
+    return PIMPC_EINVAL;
 }

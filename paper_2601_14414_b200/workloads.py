@@ -310,3 +310,25 @@ def pad_problem(p: Problem, nx2: int, nu2: int) -> Problem:
                    P=blk(p.P, nx, nx2, 1.0), Wdu=blk(p.Wdu, nu, nu2, 0.0), qbar=qbar,
                    du_lo=pad_u(p.du_lo, -1.0), du_hi=pad_u(p.du_hi, 1.0), u_prev=up, rho=p.rho, iters=p.iters,
                    tol=p.tol, dtypes=p.dtypes, meta=dict(p.meta, pad_of=(nx, nu)))
+
+
+# --------------------------------------------------------------------------------------------
+# the paper's scalability workload: random dense systems of Table I
+# --------------------------------------------------------------------------------------------
+TABLE1_SHAPES = ((10, 3), (20, 6), (30, 10), (50, 15))
+TABLE1_HORIZONS = (20, 50, 100, 200, 500)
+
+
+def paper_random(nx: int, nu: int, N: int, *, seed: int = 0, iters: int = 200) -> Problem:
+    """A, B ~ N(0, 1) with A scaled to unit spectral radius, additive disturbance e_k ~ U[-0.3, 0.3], boxes
+    |x_i| <= 5, |u_i| <= 0.1, W_y = W_u = I, W_du = 0, C = I; x0 ~ U[-1, 1].  The same (A, B) at
+    every stage (LTI, as in the paper), stored per stage like every other workload."""
+    rng = np.random.default_rng([*SEED, 7, nx, nu, seed])
+    A = rng.standard_normal((nx, nx))
+    A /= np.max(np.abs(np.linalg.eigvals(A)))
+    B = rng.standard_normal((nx, nu))
+    e = rng.uniform(-0.3, 0.3, (1, N, nx))
+    x0 = rng.uniform(-1.0, 1.0, (1, nx))
+    lo = np.concatenate([np.full(nx, -5.0), np.full(nu, -0.1)])
+    return Problem(f"T1-{nx}-{nu}-{N}", nx, nu, N, 1, np.tile(A, (1, N, 1, 1)), np.tile(B, (1, N, 1, 1)), np.eye(nx),
+                   np.eye(nu), lo, -lo, x0, e=e, rho=1.0, iters=iters, tol=0.0, dtypes=("f64", "f32"))

@@ -141,6 +141,21 @@ def test_stream_engine_all_options(oracle, pimpc, stream_grid, shape, grid, dtyp
     parity.check_properties(p, dtype, g)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("grid", [0, 3])
+@pytest.mark.parametrize("shape", [(10, 3, 17, 2), (20, 6, 9, 2), (30, 10, 7, 1), (50, 15, 5, 2)])
+def test_stream_engine_paper_table1_shapes(oracle, pimpc, stream_grid, shape, grid, dtype):
+    """The (n, m) of the paper's Table I, odd nb included (circulant storage of H without a
+    self-paired diagonal); AUTO must pick STREAM for them."""
+    nx, nu, N, batch = shape
+    stream_grid(grid)
+    p = wl.random_ltv(nx, nu, N, batch, seed=nx * 7 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
+                      qbar=True, bounds=0.8, du_bound=0.5)
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="auto", iters=100, tol=0.0)
+    assert g["info"]["engine"] == pimpc.ENGINE_STREAM
+    parity.check_properties(p, dtype, g)
+
+
 @pytest.mark.parametrize("grid", [0, 5])
 def test_stream_engine_unbounded_and_plain_admm(oracle, pimpc, stream_grid, grid):
     stream_grid(grid)
