@@ -520,7 +520,10 @@ int pimpc_reset(pimpc_t h)
 {
     int rc = check_handle(h);
     if (rc) return rc;
-    return launch_zero_state(h) < 0 ? PIMPC_ECUDA : PIMPC_OK;
+    const int n = launch_zero_state(h);
+    if (n < 0) return PIMPC_ECUDA;
+    h->info.total_launches += n;
+    return PIMPC_OK;
 }
 
 int pimpc_shift(pimpc_t h, int steps)
