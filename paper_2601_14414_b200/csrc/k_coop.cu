@@ -14,7 +14,8 @@
 //     accept / restart decision (steps 5-7).  Buffers are double-buffered on the
 //     iteration parity: a CTA cannot run two iterations ahead of a neighbour because it needs that
 //     neighbour's next partial first.
-// The launch is cooperative only to guarantee co-residency of the polling CTAs.
+// The launch is cooperative only to guarantee co-residency of the polling CTAs.  Short horizons run as ONE thread-block
+// cluster instead (template flag CL): the same tagged words are pushed into the peers' shared memory (DSMEM) and polled locally.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -41,6 +42,18 @@ template <> struct Tagged<float> {
         v = __uint_as_float(a);
         return b == tag;
     }
+    // the same word in distributed shared memory: store to a peer CTA of the cluster, poll the own CTA's copy
+    static __device__ __forceinline__ void st_cl(uint32_t raddr, float v, uint32_t tag)
+    {
+        asm volatile("st.relaxed.cluster.shared::cluster.v2.u32 [%0], {%1, %2};" ::"r"(raddr), "r"(__float_as_uint(v)), "r"(tag) : "memory");
+    }
+    static __device__ __forceinline__ bool ld_sm(const W *p, uint32_t tag, float &v)
+    {
+        uint32_t a, b;
+        asm volatile("ld.relaxed.cluster.shared::cta.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
+        v = __uint_as_float(a);
+        return b == tag;
+    }
 };
 template <> struct Tagged<double> {
     typedef uint4 W;
@@ -56,7 +69,31 @@ template <> struct Tagged<double> {
         v = __hiloint2double((int)c, (int)a);
         return b == tag && d == tag;
     }
+    static __device__ __forceinline__ void st_cl(uint32_t raddr, double v, uint32_t tag)
+    {
+        const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
+        asm volatile("st.relaxed.cluster.shared::cluster.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(raddr), "r"(lo), "r"(tag), "r"(hi), "r"(tag) : "memory");
+    }
+    static __device__ __forceinline__ bool ld_sm(const W *p, uint32_t tag, double &v)
+    {
+        uint32_t a, b, c, d;
+        asm volatile("ld.relaxed.cluster.shared::cta.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
+        v = __hiloint2double((int)c, (int)a);
+        return b == tag && d == tag;
+    }
 };
+
+// shared-memory address of the same variable in the CTA of rank `rank` of the cluster
+__device__ __forceinline__ uint32_t map_peer(const void *local, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"((uint32_t)__cvta_generic_to_shared(local)), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 
 __device__ __forceinline__ void ld4o(const float *p, float (&o)[4])
 {
@@ -89,7 +126,11 @@ struct OCfg {
     static constexpr int SSW = SSW0 + ((LPS - SSW0 % 32) + 32) % 32;
     static constexpr int SS = SSW / WPE;
     static_assert(SSW % WPE == 0 && SS % 4 == 0 && LPS <= 32 && NX % 4 == 0, "slot layout");
-    static constexpr size_t head_bytes = 40 * sizeof(double) + (KAPN + 2 * LPS + 2 * NUP) * sizeof(T);
+    // cluster variant: inbound exchange words in the CTA's own shared memory, [2 parities][CLMAX] partials of c and
+    // [2][HALO] boundary iterates ([0, 3 LPS) from the right neighbour, [3 LPS, 5 LPS) from the left one)
+    static constexpr int CLMAX = 16;
+    static constexpr size_t xpart_bytes = 2 * CLMAX * 16, xhalo_bytes = 2 * 5 * LPS * 4 * sizeof(T);
+    static constexpr size_t head_bytes = 40 * sizeof(double) + xpart_bytes + xhalo_bytes + (KAPN + 2 * LPS + 2 * NUP) * sizeof(T);
     static size_t smem_bytes(int slots) { return head_bytes + (size_t)slots * SS * sizeof(T); }
     // exchange buffers per CTA and parity (tagged words): to the left neighbour (z, v, lambda) of the first stage,
     // to the right neighbour (z, theta) of the last stage
@@ -112,7 +153,9 @@ template <typename T> struct OState { T z, v, th, be, la, d, de; };
 #define PROF_MARK(i)
 #endif
 
-template <typename T, int NX, int NU, int SPG, int MAXT, bool DU>
+// CL: the grid is ONE thread-block cluster (<= 16 CTAs) and the tagged words travel through distributed shared memory
+// (a remote store lands in ~200 cycles) instead of L2 (850-1000 cycles per hop, 2400+ for an all-to-all of 64 CTAs).
+template <typename T, int NX, int NU, int SPG, int MAXT, bool DU, bool CL>
 __global__ void __launch_bounds__(MAXT, 1)
 k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__restrict__ kappa_tab, const int iters,
        typename Tagged<double>::W *__restrict__ part, typename Tagged<T>::W *__restrict__ halo)
@@ -125,7 +168,9 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                   OAB = C::OAB, OMM = C::OMM;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double *red = reinterpret_cast<double *>(smem_raw);        // [32] warp partials, [32..33] c of the last two iterations
-    T *sKap = reinterpret_cast<T *>(red + 40);                 // [KAPN]
+    typename TD::W *xPart = reinterpret_cast<typename TD::W *>(red + 40);                         // [2][CLMAX]
+    typename TW::W *xHalo = reinterpret_cast<typename TW::W *>(smem_raw + 320 + C::xpart_bytes);  // [2][HALO]
+    T *sKap = reinterpret_cast<T *>(smem_raw + 320 + C::xpart_bytes + C::xhalo_bytes);            // [KAPN]
     T *sQ = sKap + C::KAPN;                                    // [LPS] qbar
     T *sDlo = sQ + LPS, *sDhi = sDlo + NUP;                    // [NUP] Delta-u box
     T *sBlk = sDhi + NUP + (LPS - 2 * NUP % LPS) % LPS;        // [L+2][SS]   (head_bytes reserves 2 LPS + 2 NUP)
@@ -152,6 +197,9 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         sDhi[tid] = (DU && tid < NU) ? p.dhi[tid] : (T)0;
     }
     if (tid == 0) { red[32] = p.c0; red[33] = p.c0; }
+    if (CL) {
+        for (int i = tid; i < (int)((C::xpart_bytes + C::xhalo_bytes) / 4); i += blockDim.x) reinterpret_cast<uint32_t *>(xPart)[i] = 0u;
+    }
     __syncthreads();
     for (int v = 0; v <= L + 1; ++v) {
         const int k = k0 - 1 + v;
@@ -205,6 +253,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     int jacc = 0, it_done = 0, restarts = 0;
     bool done = false;
     __syncthreads();
+    if (CL) cluster_sync_all();                  // every CTA of the cluster has zeroed its inbound words
     PROF_DECL
 
     // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.  par = it & 1.
@@ -340,12 +389,22 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             // boundary iterates for the neighbour CTAs' ghosts (tagged words, parity-double-buffered)
             const int v = s * ngroups + g;
             if (v == 1 && has_left) {
-                typename TW::W *o = halo + ((size_t)par * G + cta) * C::HALO;
-                TW::st(o + li, zn, tag); TW::st(o + LPS + li, vn, tag); TW::st(o + 2 * LPS + li, lan, tag);
+                if (CL) {
+                    const uint32_t o = map_peer(xHalo + par * C::HALO + li, cta - 1), w = sizeof(typename TW::W) * LPS;
+                    TW::st_cl(o, zn, tag); TW::st_cl(o + w, vn, tag); TW::st_cl(o + 2 * w, lan, tag);
+                } else {
+                    typename TW::W *o = halo + ((size_t)par * G + cta) * C::HALO;
+                    TW::st(o + li, zn, tag); TW::st(o + LPS + li, vn, tag); TW::st(o + 2 * LPS + li, lan, tag);
+                }
             }
             if (v == L && has_right) {
-                typename TW::W *o = halo + ((size_t)par * G + cta) * C::HALO + 3 * LPS;
-                TW::st(o + li, zn, tag); TW::st(o + LPS + li, thn, tag);
+                if (CL) {
+                    const uint32_t o = map_peer(xHalo + par * C::HALO + 3 * LPS + li, cta + 1), w = sizeof(typename TW::W) * LPS;
+                    TW::st_cl(o, zn, tag); TW::st_cl(o + w, thn, tag);
+                } else {
+                    typename TW::W *o = halo + ((size_t)par * G + cta) * C::HALO + 3 * LPS;
+                    TW::st(o + li, zn, tag); TW::st(o + LPS + li, thn, tag);
+                }
             }
         }
         // ---- step 4: c = rho * sum (fixed order: group butterfly in T, then double) ----
@@ -365,9 +424,16 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             // small grids: every CTA polls every partial (one hop).  Large grids: CTA 0 gathers, sums and publishes c
             // in NREP replicas, the others poll one replica (two hops, but 148 x 148 polls would take longer).
             typename TD::W *pp = part + (size_t)par * (G + C::NREP) * C::PSTRIDE;
-            if (lane == 0) TD::st(pp + (size_t)cta * C::PSTRIDE, sum, tag);
             const bool a2a = G <= C::A2A_MAX;
-            if (a2a || cta == 0) {
+            if (CL) {                                  // push the partial into every CTA of the cluster, poll the own copies
+                if (lane < G) TD::st_cl(map_peer(xPart + par * C::CLMAX + cta, lane), sum, tag);
+                double val = 0.0;
+                if (lane < G) while (!TD::ld_sm(xPart + par * C::CLMAX + lane, tag, val)) {}
+                sum = val;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            } else if (a2a || cta == 0) {
+                if (lane == 0) TD::st(pp + (size_t)cta * C::PSTRIDE, sum, tag);
                 double vals[C::MAXJ];
                 bool got[C::MAXJ];
 #pragma unroll
@@ -387,6 +453,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
                 if (!a2a && lane < C::NREP) TD::st(pp + (size_t)(G + lane) * C::PSTRIDE, sum, tag);
             } else {
+                if (lane == 0) TD::st(pp + (size_t)cta * C::PSTRIDE, sum, tag);
                 if (lane == 0) while (!TD::ld(pp + (size_t)(G + cta % C::NREP) * C::PSTRIDE, tag, sum)) {}
                 sum = __shfl_sync(0xffffffffu, sum, 0);
             }
@@ -396,20 +463,23 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 #pragma unroll
             for (int s = 0; s < SPG; ++s) {
                 if (ghl[s] && rowok) {
-                    const typename TW::W *o = halo + ((size_t)par * G + cta - 1) * C::HALO + 3 * LPS;
+                    const typename TW::W *o = CL ? xHalo + par * C::HALO + 3 * LPS : halo + ((size_t)par * G + cta - 1) * C::HALO + 3 * LPS;
                     T a, b2;
                     bool ga = false, gb = false;
-                    do { if (!ga) ga = TW::ld(o + li, tag, a); if (!gb) gb = TW::ld(o + LPS + li, tag, b2); } while (!(ga && gb));
+                    do {
+                        if (!ga) ga = CL ? TW::ld_sm(o + li, tag, a) : TW::ld(o + li, tag, a);
+                        if (!gb) gb = CL ? TW::ld_sm(o + LPS + li, tag, b2) : TW::ld(o + LPS + li, tag, b2);
+                    } while (!(ga && gb));
                     prv[s].z = a; prv[s].th = b2;
                 }
                 if (ghr[s] && rowok) {
-                    const typename TW::W *o = halo + ((size_t)par * G + cta + 1) * C::HALO;
+                    const typename TW::W *o = CL ? xHalo + par * C::HALO : halo + ((size_t)par * G + cta + 1) * C::HALO;
                     T a, b2, c2;
                     bool ga = false, gb = false, gc = false;
                     do {
-                        if (!ga) ga = TW::ld(o + li, tag, a);
-                        if (!gb) gb = TW::ld(o + LPS + li, tag, b2);
-                        if (!gc) gc = TW::ld(o + 2 * LPS + li, tag, c2);
+                        if (!ga) ga = CL ? TW::ld_sm(o + li, tag, a) : TW::ld(o + li, tag, a);
+                        if (!gb) gb = CL ? TW::ld_sm(o + LPS + li, tag, b2) : TW::ld(o + LPS + li, tag, b2);
+                        if (!gc) gc = CL ? TW::ld_sm(o + 2 * LPS + li, tag, c2) : TW::ld(o + 2 * LPS + li, tag, c2);
                     } while (!(ga && gb && gc));
                     prv[s].z = a; prv[s].v = b2; prv[s].la = c2;
                 }
@@ -473,15 +543,21 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         c.done = done ? 1 : 0; c.iters = it_done; c.restarts = restarts;
         p.ctl[0] = c;
     }
+    if (CL) cluster_sync_all();                  // no CTA leaves while a peer could still address its shared memory
 }
 
-struct CoopPlan { int grid, spg, threads, slots; size_t smem; };
+struct CoopPlan { int grid, spg, threads, slots; size_t smem; int cluster; };
 
 int env_int_o(const char *name, int dflt)
 {
     const char *v = getenv(name);
     return v && *v ? atoi(v) : dflt;
 }
+
+// Horizons up to this length run as ONE cluster of 16 CTAs (B200, C3 generator, us per iteration, cluster vs 64 CTAs over
+// L2: fp32 N=100 1.24 / 2.34, 200 1.42 / 2.25, 400 1.83 / 2.58, 700 2.57 / 2.55; fp64 N=100 1.56 / 2.45, 200 1.91 / 2.57,
+// 400 2.75 / 2.70); beyond it the ranges per CTA get too long and more CTAs exchanging through L2 win.
+constexpr int CL_MAXN_F32 = 600, CL_MAXN_F64 = 350;
 
 template <typename T, int NX, int NU>
 bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
@@ -490,8 +566,13 @@ bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
     const int gmax = std::min(h->sm_count, 32 * C::MAXJ);
     // ranges of >= 16 stages until 64 CTAs are busy, then as many CTAs as SMs (measured: the exchange grows with the grid)
     int grid = std::min(gmax, std::max((h->N + 15) / 16, std::min(h->N, 64)));
+    // short horizons: ONE cluster of <= 16 CTAs exchanging through distributed shared memory (PIMPC_COOP_CLUSTER = 0
+    // disables, = n forces n CTAs; default 16 while N <= CL_MAXN)
+    const int cl_env = env_int_o("PIMPC_COOP_CLUSTER", -1);
+    int cluster = cl_env >= 0 ? std::min(cl_env, C::CLMAX) : (h->N <= (sizeof(T) == 4 ? CL_MAXN_F32 : CL_MAXN_F64) ? C::CLMAX : 0);
+    if (cluster > 0) { cluster = std::min(cluster, h->N); grid = cluster; }
     const int gforce = env_int_o("PIMPC_COOP_GRID", 0);        // test hook: fewer CTAs = longer ranges per CTA
-    if (gforce > 0) grid = std::min(grid, gforce);
+    if (gforce > 0) { grid = std::min(grid, gforce); if (cluster) cluster = grid; }
     const int L = (h->N + grid - 1) / grid;                    // longest range
     const int slots = L + 2, gpw = 32 / C::LPS;
     const int spg_max = sizeof(T) == 8 ? 1 : 2;
@@ -501,7 +582,7 @@ bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
     const int ncw = ((slots + spg - 1) / spg + gpw - 1) / gpw;
     const size_t smem = C::smem_bytes(slots);
     if (smem > h->smem_optin) { if (why) *why = "stage matrices of a CTA's range do not fit in shared memory"; return false; }
-    pl->grid = grid; pl->spg = spg; pl->threads = (ncw + 1) * 32; pl->slots = slots; pl->smem = smem;
+    pl->grid = grid; pl->spg = spg; pl->threads = (ncw + 1) * 32; pl->slots = slots; pl->smem = smem; pl->cluster = cluster;
     return true;
 }
 
@@ -511,7 +592,28 @@ int launch_coop(pimpc_s *h, int iters, double tol, const CoopPlan &pl)
     using C = OCfg<T, NX, NU>;
     typedef typename Tagged<double>::W PW;
     typedef typename Tagged<T>::W HW;
-    auto kern = h->has_du ? k_coop<T, NX, NU, SPG, MAXT, true> : k_coop<T, NX, NU, SPG, MAXT, false>;
+    if (pl.cluster > 0) {
+        // one thread-block cluster: co-scheduled by the hardware, exchange through distributed shared memory
+        auto kc = h->has_du ? k_coop<T, NX, NU, SPG, MAXT, true, true> : k_coop<T, NX, NU, SPG, MAXT, false, true>;
+        PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(kc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.cluster > 8) PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(kc, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(pl.grid); cfg.blockDim = dim3(pl.threads); cfg.dynamicSmemBytes = pl.smem; cfg.stream = h->stream;
+        cudaLaunchAttribute at1[1];
+        at1[0].id = cudaLaunchAttributeClusterDimension;
+        at1[0].val.clusterDim.x = pl.grid; at1[0].val.clusterDim.y = 1; at1[0].val.clusterDim.z = 1;
+        cfg.attrs = at1; cfg.numAttrs = 1;
+        int ncl = 0;
+        if (cudaOccupancyMaxActiveClusters(&ncl, kc, &cfg) == cudaSuccess && ncl >= 1) {
+            Prob<T> pc = make_prob<T>(h, tol);
+            const double *atc = h->alpha_tab, *ktc = h->kappa_tab;
+            PIMPC_CUDA_TRY(h, cudaLaunchKernelEx(&cfg, kc, pc, atc, ktc, iters, (PW *)nullptr, (HW *)nullptr));
+            h->info.grid = pl.grid; h->info.block = pl.threads; h->info.smem_bytes = pl.smem;
+            return 1;
+        }
+        cudaGetLastError();                      // no room for such a cluster: the L2 path below with the same plan
+    }
+    auto kern = h->has_du ? k_coop<T, NX, NU, SPG, MAXT, true, false> : k_coop<T, NX, NU, SPG, MAXT, false, false>;
     PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     int occ = 0;
     PIMPC_CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, pl.smem));

@@ -187,25 +187,30 @@ def test_stream_engine_early_stop_and_warm_start(oracle, pimpc, stream_grid, gri
 # ---- COOP engine (batch 1, horizon spread over the SMs, tagged-word exchange instead of grid barriers) ------
 @pytest.fixture
 def coop_env(monkeypatch):
-    def set_(grid=0, spg=0):
+    def set_(grid=0, spg=0, cluster=None):
         for name, v in (("PIMPC_COOP_GRID", grid), ("PIMPC_COOP_SPG", spg)):
             if v:
                 monkeypatch.setenv(name, str(v))
             else:
                 monkeypatch.delenv(name, raising=False)
+        if cluster is None:                       # default: one cluster (DSMEM exchange) for short horizons
+            monkeypatch.delenv("PIMPC_COOP_CLUSTER", raising=False)
+        else:                                     # 0: exchange through L2 (the long-horizon path); n: cluster of n CTAs
+            monkeypatch.setenv("PIMPC_COOP_CLUSTER", str(cluster))
     return set_
 
 
+@pytest.mark.parametrize("cluster", [None, 0, 8])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("grid", [0, 1, 2, 7])
 @pytest.mark.parametrize("shape", [(12, 4, 41), (4, 2, 23), (12, 4, 150), (4, 2, 1), (12, 4, 2)])
-def test_coop_engine_all_options(oracle, pimpc, coop_env, shape, grid, dtype):
+def test_coop_engine_all_options(oracle, pimpc, coop_env, shape, grid, dtype, cluster):
     """grid = 0: one stage per CTA while N <= 148 (every stage has two ghosts); 1: a single CTA, no exchange;
     2, 7: ragged ranges.  All optional terms on."""
     nx, nu, N = shape
     if N > 100 and grid in (1, 2):
         grid += 4                         # 150 stages of (12, 4) do not fit one or two CTAs' shared memory: 5, 6 CTAs
-    coop_env(grid)
+    coop_env(grid, cluster=cluster)
     p = wl.random_ltv(nx, nu, N, 1, seed=nx * 10 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
                       qbar=True, bounds=0.8, du_bound=0.5)
     g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="coop", iters=120, tol=0.0)
@@ -213,17 +218,19 @@ def test_coop_engine_all_options(oracle, pimpc, coop_env, shape, grid, dtype):
     parity.check_properties(p, dtype, g)
 
 
+@pytest.mark.parametrize("cluster", [None, 0])
 @pytest.mark.parametrize("grid", [3, 0])
-def test_coop_engine_two_stages_per_group_fp32(oracle, pimpc, coop_env, grid):
-    coop_env(grid, spg=2)
+def test_coop_engine_two_stages_per_group_fp32(oracle, pimpc, coop_env, grid, cluster):
+    coop_env(grid, spg=2, cluster=cluster)
     p = wl.random_ltv(12, 4, 100, 1, seed=5, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
     g, worst, nrep = parity.check(oracle, pimpc, p, "f32", engine="coop", iters=150, tol=0.0)
     assert g["info"]["engine"] == pimpc.ENGINE_COOP
 
 
+@pytest.mark.parametrize("cluster", [None, 0])
 @pytest.mark.parametrize("grid", [0, 5])
-def test_coop_engine_unbounded_plain_admm_early_stop_warm_start(oracle, pimpc, coop_env, grid):
-    coop_env(grid)
+def test_coop_engine_unbounded_plain_admm_early_stop_warm_start(oracle, pimpc, coop_env, grid, cluster):
+    coop_env(grid, cluster=cluster)
     p = wl.random_ltv(4, 2, 9, 1, seed=77, affine=True, bounds=None, du_bound=None)
     g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="coop", iters=300, tol=0.0)
     assert "D" not in g
