@@ -69,6 +69,7 @@ def ncu_traffic(engine, config):
 
 
 def alu_peak_tflops(dtype, sm_mhz, sms=148):
+    """Nominal FMA peak (lanes x 2 x clock), quoted next to the MEASURED one of pimpc_measure_peaks."""
     lanes = 128 if dtype == "f32" else 64          # FP32 / FP64 FMA lanes per SM (DESIGN.md)
     return sms * lanes * 2 * sm_mhz * 1e6 / 1e12
 
@@ -262,7 +263,8 @@ def extras(torch, pimpc, pk):
         balg = bytes_per_stage_iter(p5.nx, p5.nu, esz) * p5.N * p5.batch
         out[f"C5_{dt}"] = {"ms_per_iter": ms_it, "algorithmic_GBps": balg / ms_it / 1e6,
                            "frac_of_hbm_peak": balg / ms_it / 1e6 / pk["hbm_gbs"], "engine": info["engine"],
-                           "solves_per_s_500it": p5.batch / (ms_it * 500 / 1e3)}
+                           "solves_per_s_500it_iterations_only": p5.batch / (ms_it * 500 / 1e3),
+                           "note": "iteration kernel only: excludes the a0 cache kernel and k_pack"}
         s.close()
     return out
 
@@ -303,7 +305,8 @@ def main():
     x_h = torch.empty(BATCH, prob.N, prob.nx, dtype=f32).pin_memory()
     u_h = torch.empty(BATCH, prob.N, prob.nu, dtype=f32).pin_memory()
     du_h = torch.empty(BATCH, prob.N, prob.nu, dtype=f32).pin_memory()
-    res_h = torch.zeros(BATCH, 32, dtype=torch.uint8).pin_memory()
+    res_h = torch.zeros(BATCH, pimpc.RESULT_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
+    onchip = pimpc.measure_peaks(torch.cuda.current_stream().cuda_stream)     # FMA-chain / smem microbenchmarks, untimed
 
     s = pimpc.Solver(prob.nx, prob.nu, prob.N, BATCH, dtype="f32", engine=args.engine, rho=prob.rho)
     s.set_cost(prob.Q, prob.R)
@@ -315,22 +318,35 @@ def main():
         info = s.get_info()                    # waits for the solve; device times of the two kernels
         iter_ms.append(info["iter_ms"]); setup_ms.append(info["setup_ms"])
 
-    # e2e: the calls a user makes, pinned host buffers in and out.  Two handles of half the batch on two streams:
-    # the H2D copy / D2H read of one half overlaps the solve of the other (instances are independent).
-    half = BATCH // 2
+    # e2e: the calls a user makes, pinned host buffers in and out.  The batch is cut into slices of whole waves of CTAs
+    # (a multiple of the SM count instances each; instances are independent), one handle and stream per slice, and the
+    # loop is software-pipelined: as soon as a slice's results of step i have been read back, its inputs of step i+1 are
+    # enqueued, so every step's H2D / D2H copies (all inside the timed region) overlap the other slices' solves.
+    sms = s.get_info()["sm_count"]
+    per = -(-BATCH // (7 * sms)) * sms
+    cuts = [(a, min(a + per, BATCH)) for a in range(0, BATCH, per)]
     pair = []
-    for sl in (slice(0, half), slice(half, BATCH)):
-        h = pimpc.Solver(prob.nx, prob.nu, prob.N, sl.stop - sl.start, dtype="f32", engine=args.engine, rho=prob.rho,
+    for a, b_ in cuts:
+        h = pimpc.Solver(prob.nx, prob.nu, prob.N, b_ - a, dtype="f32", engine=args.engine, rho=prob.rho,
                          stream=torch.cuda.Stream().cuda_stream)
         h.set_cost(prob.Q, prob.R)
         h.set_bounds(prob.lo, prob.hi, prob.du_lo, prob.du_hi)
-        pair.append((h, sl))
+        pair.append((h, slice(a, b_)))
 
-    def step_e2e():
+    def e2e_issue(h, sl):
+        h.set_stages(A_h[sl], B_h[sl]); h.set_x0(x0_h[sl]); h.reset(); h.solve(ITERS)
+
+    def e2e_collect(h, sl):
+        h.get(x_h[sl], u_h[sl], du_h[sl], res_h[sl])
+
+    def e2e_steps(k):
         for h, sl in pair:
-            h.set_stages(A_h[sl], B_h[sl]); h.set_x0(x0_h[sl]); h.reset(); h.solve(ITERS)
-        for h, sl in pair:
-            h.get(x_h[sl], u_h[sl], du_h[sl], res_h[sl])
+            e2e_issue(h, sl)
+        for step in range(k):
+            for h, sl in pair:
+                e2e_collect(h, sl)
+                if step + 1 < k:
+                    e2e_issue(h, sl)
 
     for _ in range(args.warmup):
         step_resident()
@@ -349,10 +365,15 @@ def main():
     ms = replicas.max_over_ranks(ms, local_rank)
     info = s.get_info()
 
-    for _ in range(max(1, args.warmup // 2)):
-        step_e2e()
+    e2e_steps(max(1, args.warmup // 2))
     replicas.barrier(local_rank)
-    ms_e2e = timed_loop(torch, args.steps, step_e2e)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()                               # the slices run on their own streams: events bracket full device syncs
+    e2e_steps(args.steps)
+    torch.cuda.synchronize()
+    ev1.record(); ev1.synchronize()
+    ms_e2e = ev0.elapsed_time(ev1)
     replicas.barrier(local_rank)
     ms_e2e = replicas.max_over_ranks(ms_e2e, local_rank)
     res = np.frombuffer(res_h.numpy().tobytes(), dtype=pimpc.RESULT_DTYPE)
@@ -369,12 +390,15 @@ def main():
                 "kernel": "STAGED engine: 5 kernels per iteration (k_hat,k_adj,k_primal,k_dual,k_decide)", "traffic": None}
     else:
         fl = flops_per_stage_iter(prob.nx, prob.nu) * nst * ITERS
-        roof = {"bound": "alu", "achieved": fl / k_ms / 1e9, "peak": alu_peak_tflops("f32", pk["sm_max_mhz"]),
+        roof = {"bound": "alu", "achieved": fl / k_ms / 1e9, "peak": onchip["ffma2_tflops"],
                 "unit": "TFLOP/s", "kernel": "k_resident<float,12,4> (one persistent launch per solve)", "traffic": None,
+                "peak_nominal": alu_peak_tflops("f32", pk["sm_max_mhz"]), "measured_onchip_peaks": onchip,
                 "algorithmic_GBps_if_streamed": bytes_per_stage_iter(prob.nx, prob.nu, 4) * nst * ITERS / k_ms / 1e6}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["peak_source"] = ("MEASURED_PEAKS.json" if pk["source"] == "measured" else "fallback") + \
-        (" hbm_gbs" if roof["bound"] == "hbm" else " sm_max_mhz x 148 SM x 128 FP32 lanes x 2 (DESIGN.md)")
+    roof["peak_source"] = ("MEASURED_PEAKS.json hbm_gbs" if pk["source"] == "measured" else "fallback hbm_gbs") \
+        if roof["bound"] == "hbm" else \
+        "pimpc_measure_peaks(): packed-FFMA2 dependency-chain microbenchmark run on this GPU just before the timed region " \
+        "(the FMA pipe binds: DESIGN.md section 6; shared-memory peak in measured_onchip_peaks)"
     roof["kernel_ms_per_launch"] = k_ms
     roof["cache_kernel_ms"] = statistics.mean(setup_ms)
     roof["traffic"] = ncu_traffic(engine, "C4_f32")
@@ -388,7 +412,8 @@ def main():
         "config": workload_config(world),
         "e2e": {"value": world * BATCH * args.steps / (ms_e2e / 1e3), "unit": "solves/s", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps,
-                "how": "two handles x 2048 instances on two streams, pinned host buffers, copies overlap the other half's solve"},
+                "how": f"{len(pair)} handles x {per} instances (whole waves of {sms} CTAs) on their own streams, pinned host "
+                       "buffers, software-pipelined: a slice's next inputs are enqueued right after its results were read"},
         "gpu_launches": int(launches), "clocks": ck, "roofline": roof,
         "engine": {1: "staged", 2: "resident", 3: "stream", 4: "coop"}.get(engine, str(engine)),
         "iterations_per_s": world * BATCH * ITERS * args.steps / (ms / 1e3),

@@ -50,6 +50,22 @@ enum {
 enum { PIMPC_X = 0, PIMPC_Z = 1, PIMPC_V = 2, PIMPC_TH = 3, PIMPC_BE = 4, PIMPC_LA = 5, PIMPC_D = 6,
        PIMPC_DE = 7, PIMPC_DU = 8 };
 
+/* Launch-shape overrides of the fused engines; 0 everywhere = automatic (what pimpc_default_opts sets).  They do not
+ * change WHAT is computed, only how the stages are spread over CTAs / lanes; the parity tests use them to reach every
+ * code path (ranges that split instances, ragged ranges, single-CTA runs) on small problems. */
+typedef struct {
+    int grid;             /* STREAM, COOP: at most this many CTAs (fewer CTAs = longer stage ranges per CTA)       */
+    int ctas_per_sm;      /* STREAM: resident CTAs per SM                                                          */
+    int ring_slots;       /* STREAM: at most this many slots in the bulk-copy ring                                 */
+    int stages_per_group; /* COOP: stages per lane group (1 or 2)                                                  */
+    int cluster;          /* COOP: -1 = never one thread-block cluster (exchange through L2), n > 0 = cluster of
+                             n CTAs (<= 16), 0 = automatic (one cluster for short horizons)                       */
+    int rows_per_lane;    /* RESIDENT: matrix rows per lane (1 or 2; 2 only where instantiated)                    */
+    int lookahead;        /* COOP: 1 = prepare the next iteration for both candidate momenta while the partial sums
+                             of c travel, -1 = never, 0 = automatic                                 */
+    int reserved_;
+} pimpc_tune;
+
 typedef struct {
     int dtype;        /* PIMPC_F64 | PIMPC_F32: arithmetic and I/O element type                      */
     int engine;       /* PIMPC_ENGINE_*; AUTO = 0                                                     */
@@ -58,12 +74,21 @@ typedef struct {
     double c0;        /* c^0; 0 -> 1.0                                             */
     int history;      /* > 0: keep (c^{i+1}, accept bit) of up to `history` iterations per instance   */
     void *stream;     /* cudaStream_t on which all work of the handle is enqueued                     */
+    void *workspace;  /* DEVICE memory for the handle's problem data, cache and iterates, or NULL: the library
+                         allocates.  256-byte aligned, at least pimpc_workspace_bytes() bytes, owned by the caller
+                         and kept alive until pimpc_destroy.  Engine-private scratch that depends on the launch
+                         plan (packed blobs, exchange words, result staging) is always allocated by the library. */
+    size_t workspace_bytes; /* size of `workspace`; EINVAL if it is given and too small                */
+    pimpc_tune tune;  /* launch-shape overrides, all 0 = automatic                                    */
 } pimpc_opts;
 
 /* Per-instance result record written by pimpc_get (always double/int, host or device). */
 typedef struct {
     double c;         /* c^{i+1} of the last executed iteration                    */
     double alpha;     /* alpha after the last decision                             */
+    double r_prim2;   /* rho ||F p + G q - h||^2 of the returned iterate: the primal-residual half of c
+                         ((14a), (15c)), evaluated from its definition on X, DU, Z, V[, D]  */
+    double r_dual2;   /* c - r_prim2 = rho ||G (q^{i+1} - qhat^i)||^2, the dual-residual half  */
     int iters;        /* iterations executed (i+1 at the break of step 5, else max_iters)             */
     int restarts;     /* number of times step 7 (restart) was taken                                   */
     int converged;    /* 1 if step 5 (c < tol) stopped the instance                                   */
@@ -83,18 +108,36 @@ typedef struct {
                                  the handle's stream; pimpc_get_info waits for them)                  */
 } pimpc_info;
 
+/* On-chip peaks of the current device, MEASURED by dependency-chain microbenchmarks (a few tens of milliseconds each):
+ * the rooflines the register-resident engine is reported against ("measure both with an FMA-chain
+ * microbenchmark ... declare which one binds").  TFLOP/s count 2 flops per FMA. */
+typedef struct {
+    double ffma_tflops;   /* scalar fma.rn.f32                                                          */
+    double ffma2_tflops;  /* packed fma.rn.f32x2 (what the fp32 mat-vecs of the RESIDENT engine issue)  */
+    double dfma_tflops;   /* fma.rn.f64                                                                 */
+    double smem_gbs;      /* conflict-free 16-byte shared-memory loads, all SMs                         */
+    int sm_count;
+    int pad_;
+} pimpc_peaks;
+
 const char *pimpc_version(void);
 
-/* Fill `o` with defaults (f64, AUTO, rho=1, eta=0.999, c0=1, no history, default stream). */
+/* Run the microbenchmarks on the current device and `stream` (a cudaStream_t, NULL = default); synchronises.
+ * EINVAL: out is NULL; ECUDA / ENOMEM on device errors. */
+int pimpc_measure_peaks(pimpc_peaks *out, void *stream);
+
+/* Fill `o` with defaults (f64, AUTO, rho=1, eta=0.999, c0=1, no history, default stream, no workspace, tune = 0). */
 void pimpc_default_opts(pimpc_opts *o);
 
-/* Device bytes pimpc_create would allocate for these dimensions (0 on invalid arguments). */
+/* Device bytes pimpc_create allocates for these dimensions = the size a caller-provided opts.workspace must have
+ * (0 on invalid arguments). */
 size_t pimpc_workspace_bytes(int nx, int nu, int N, int batch, const pimpc_opts *opts);
 
 /* Create a solver for `batch` independent MPC instances with nx states, nu inputs, horizon N
  * (Problem (1)).  Cold start (all iterates 0, reading R9), e_k = 0, qbar = 0,
  * u_prev = 0, no bounds (+-inf), Q = I, R = I until the setters are called.
- * opts may be NULL (defaults).  EINVAL: nx,nu,N,batch <= 0, nx+nu > 128, rho <= 0, bad dtype. */
+ * opts may be NULL (defaults).  EINVAL: nx,nu,N,batch <= 0, nx+nu > 160, batch > 65535, rho <= 0, bad dtype,
+ * workspace too small or misaligned. */
 int pimpc_create(pimpc_t *out, int nx, int nu, int N, int batch, const pimpc_opts *opts);
 int pimpc_destroy(pimpc_t h);
 

@@ -127,6 +127,9 @@ static double sq(double x) { return x * x; }
  *       c^{i+1} and the decision bit of iteration i (bit = 0 for the stopping iteration)
  *   info[0] = iterations executed, info[1] = number of restarts (step 7 taken)
  *   c_last = c of the last executed iteration
+ *   r_parts [2] or NULL: the two halves of c_last:
+ *       r_parts[0] = rho ||s^{i+1} - shat^i||^2  (primal residual F p + G q - h, by (15c))
+ *       r_parts[1] = rho ||G (q^{i+1} - qhat^i)||^2  (dual residual)
  * Returns 0, -1 bad argument, -2 out of memory, -5 matrix not positive definite.
  */
 int pimpc_oracle_solve(
@@ -142,7 +145,7 @@ int pimpc_oracle_solve(
     double *Z, double *V, double *TH, double *BE, double *LA, double *D, double *DE,
     double *X, double *DU,
     double *c_hist, unsigned char *acc_hist,
-    int *info, double *c_last)
+    int *info, double *c_last, double *r_parts)
 {
     if (nx <= 0 || nu <= 0 || N <= 0 || !(rho > 0.0) || max_iters < 0) return -1;
     if ((du_lo == NULL) != (du_hi == NULL)) return -1;
@@ -239,7 +242,7 @@ int pimpc_oracle_solve(
     memcpy(THh, TH, szb * sizeof(double)); memcpy(BEh, BE, szb * sizeof(double));
     memcpy(LAh, LA, szb * sizeof(double));
     if (has_du) { memcpy(Dh, D, szu * sizeof(double)); memcpy(DEh, DE, szu * sizeof(double)); }
-    double alpha = 1.0, c_prev = c0, c = c0;
+    double alpha = 1.0, c_prev = c0, c = c0, rp = 0.0, rd = 0.0;
     int iters = 0, restarts = 0;
 
     for (int it = 0; it < max_iters; ++it) {
@@ -266,7 +269,7 @@ int pimpc_oracle_solve(
             matvec(nb, nb, H + (size_t)k * nb * nb, t3, X + (size_t)k * nb);   /* xbar_{k+1} = H_k h_k */
         }
         /* ---- steps 2, 3 (Thm 1 proof PAPER.md:150-164, R1) and 4 (R7) ---- */
-        double csum = 0.0;
+        double csum = 0.0, psum = 0.0, dsum = 0.0;
         for (int k = 0; k < N; ++k) {
             const double *Ab = Abar + (size_t)k * nb * nb, *Bb = Bbar + (size_t)k * nb * nu;
             const double *xk = (k == 0) ? xbar0 : X + (size_t)(k - 1) * nb;    /* xbar_k^{i+1} */
@@ -285,6 +288,8 @@ int pimpc_oracle_solve(
                 LAn[q] = zn - b - vn;                          /* = lambdahat + z - Abar xbar - v - ebar */
                 csum += sq(THn[q] - THh[q]) + sq(BEn[q] - BEh[q]) + sq(LAn[q] - LAh[q])
                       + sq(zn - Zh[q]) + sq(vn - Vh[q]) + sq((zn - vn) - (Zh[q] - Vh[q]));
+                psum += sq(THn[q] - THh[q]) + sq(BEn[q] - BEh[q]) + sq(LAn[q] - LAh[q]);        /* ||Delta s||^2   */
+                dsum += sq(zn - Zh[q]) + sq(vn - Vh[q]) + sq((zn - vn) - (Zh[q] - Vh[q]));      /* ||G Delta q||^2 */
             }
             if (has_du) {                                      /* R12 */
                 for (int i = 0; i < nu; ++i) {
@@ -293,10 +298,13 @@ int pimpc_oracle_solve(
                     Dn[q] = dn;
                     DEn[q] = DEh[q] + DU[q] - dn;
                     csum += sq(DEn[q] - DEh[q]) + sq(dn - Dh[q]);
+                    psum += sq(DEn[q] - DEh[q]);
+                    dsum += sq(dn - Dh[q]);
                 }
             }
         }
         c = rho * csum;
+        rp = rho * psum; rd = rho * dsum;
         iters = it + 1;
         if (c_hist) c_hist[it] = c;
 
@@ -341,6 +349,7 @@ int pimpc_oracle_solve(
     }
     if (info) { info[0] = iters; info[1] = restarts; }
     if (c_last) *c_last = c;
+    if (r_parts) { r_parts[0] = rp; r_parts[1] = rd; }
 
 done:
     free(Abar); free(Bbar); free(ebar); free(Qbar); free(QbarN); free(qb); free(xbar0);

@@ -37,7 +37,7 @@ def _load():
         _lib.pimpc_oracle_solve.restype = ctypes.c_int
         _lib.pimpc_oracle_solve.argtypes = (
             [ctypes.c_int] * 3 + [dp] * 14 + [ctypes.c_double] * 3 + [ctypes.c_int, ctypes.c_double]
-            + [dp, ctypes.c_int] + [dp] * 9 + [dp, dp] + [dp, dp])
+            + [dp, ctypes.c_int] + [dp] * 9 + [dp, dp] + [dp, dp, dp])
         _lib.pimpc_oracle_cache.restype = ctypes.c_int
         _lib.pimpc_oracle_cache.argtypes = (
             [ctypes.c_int] * 3 + [dp] * 6 + [ctypes.c_int, ctypes.c_double] + [dp, dp])
@@ -73,6 +73,8 @@ class OracleResult:
     iters: int
     restarts: int
     c_last: float
+    r_prim2: float = 0.0                  # rho ||F p + G q - h||^2 half of c_last
+    r_dual2: float = 0.0                  # rho ||G (q - qhat)||^2 half of c_last
     x: np.ndarray = field(default=None)   # x_1..x_N  = Z[:, :nx]  (bound-feasible copy)
     u: np.ndarray = field(default=None)   # u_0..u_{N-1} = Z[:, nx:]
 
@@ -100,7 +102,7 @@ def solve(A, B, Q, R, lo, hi, x0, *, e=None, P=None, Wdu=None, qbar=None, du_lo=
             st[name] = np.zeros((N, w))
     X = np.zeros((N, nb)); DU = np.zeros((N, nu))
     c_hist = np.zeros(max(max_iters, 1)); acc_hist = np.zeros(max(max_iters, 1), dtype=np.uint8)
-    info = np.zeros(2, dtype=np.int32); c_last = np.zeros(1)
+    info = np.zeros(2, dtype=np.int32); c_last = np.zeros(1); r_parts = np.zeros(2)
     if forced is not None:
         forced = np.ascontiguousarray(np.asarray(forced, dtype=np.uint8))
     rc = lib.pimpc_oracle_solve(
@@ -109,7 +111,7 @@ def solve(A, B, Q, R, lo, hi, x0, *, e=None, P=None, Wdu=None, qbar=None, du_lo=
         float(rho), float(eta), float(c0), int(max_iters), float(tol),
         _p(forced), 0 if forced is None else int(forced.size),
         _p(st["Z"]), _p(st["V"]), _p(st["TH"]), _p(st["BE"]), _p(st["LA"]), _p(st["D"]), _p(st["DE"]),
-        _p(X), _p(DU), _p(c_hist), _p(acc_hist), _p(info), _p(c_last))
+        _p(X), _p(DU), _p(c_hist), _p(acc_hist), _p(info), _p(c_last), _p(r_parts))
     if rc != 0:
         raise RuntimeError(f"pimpc_oracle_solve failed: {rc}")
     it = int(info[0])
@@ -117,7 +119,7 @@ def solve(A, B, Q, R, lo, hi, x0, *, e=None, P=None, Wdu=None, qbar=None, du_lo=
         X=X, DU=DU, Z=st["Z"], V=st["V"], TH=st["TH"], BE=st["BE"], LA=st["LA"],
         D=st["D"] if has_du else None, DE=st["DE"] if has_du else None,
         c_hist=c_hist[:it].copy(), acc_hist=acc_hist[:it].copy(), iters=it, restarts=int(info[1]),
-        c_last=float(c_last[0]), x=st["Z"][:, :nx].copy(), u=st["Z"][:, nx:].copy())
+        c_last=float(c_last[0]), r_prim2=float(r_parts[0]), r_dual2=float(r_parts[1]), x=st["Z"][:, :nx].copy(), u=st["Z"][:, nx:].copy())
 
 
 def cache(A, B, Q, R, *, P=None, Wdu=None, has_du=False, rho=1.0):

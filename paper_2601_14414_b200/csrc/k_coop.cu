@@ -17,8 +17,6 @@
 // The launch is cooperative only to guarantee co-residency of the polling CTAs.  Short horizons run as ONE thread-block
 // cluster instead (template flag CL): the same tagged words are pushed into the peers' shared memory (DSMEM) and polled locally.
 #include <algorithm>
-#include <cstdio>
-#include <cstdlib>
 
 #include "pimpc_internal.h"
 
@@ -27,59 +25,67 @@ namespace {
 __host__ __device__ constexpr int pow2ceil_o(int v) { int p = 1; while (p < v) p <<= 1; return p; }
 __host__ __device__ constexpr int round4_o(int v) { return (v + 3) / 4 * 4; }
 
-// ---- tagged words: {value bits, tag}; 8-byte parts are single-copy atomic, each part carries its own tag ----
+// ---- tagged words: {value bits, iteration tag} in ONE 64-bit scalar access --------------------------------------
+// The PTX memory model makes a scalar .b64 access single-copy atomic, so a reader can never pair a new tag with old
+// value bits (a .v2.u32 access is two independent 32-bit accesses by specification).  fp32: one word {value, tag};
+// fp64: two such words {lo, tag}, {hi, tag}, each atomic on its own, both tags must match.
+// Ordering: a word is self-validating (the tag travels with the value), so no fence orders it against other words.
+// Reuse of a parity buffer two iterations later is safe because the writer of iteration i+2 has consumed the partial
+// sum of c of iteration i+1 from every CTA, which each CTA publishes only after its own reads of iteration i are done
+// (program order through the CTA barrier between the ghost reads and the next phase D).
+__device__ __forceinline__ uint64_t tw_pack(uint32_t v, uint32_t tag) { return (uint64_t)v | ((uint64_t)tag << 32); }
 template <typename T> struct Tagged;
 template <> struct Tagged<float> {
-    typedef uint2 W;
+    typedef uint64_t W;
     static __device__ __forceinline__ void st(W *p, float v, uint32_t tag)
     {
-        asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(__float_as_uint(v)), "r"(tag) : "memory");
+        asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(tw_pack(__float_as_uint(v), tag)) : "memory");
     }
     static __device__ __forceinline__ bool ld(const W *p, uint32_t tag, float &v)
     {
-        uint32_t a, b;
-        asm volatile("ld.relaxed.gpu.global.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "l"(p) : "memory");
-        v = __uint_as_float(a);
-        return b == tag;
+        uint64_t w;
+        asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(w) : "l"(p) : "memory");
+        v = __uint_as_float((uint32_t)w);
+        return (uint32_t)(w >> 32) == tag;
     }
     // the same word in distributed shared memory: store to a peer CTA of the cluster, poll the own CTA's copy
     static __device__ __forceinline__ void st_cl(uint32_t raddr, float v, uint32_t tag)
     {
-        asm volatile("st.relaxed.cluster.shared::cluster.v2.u32 [%0], {%1, %2};" ::"r"(raddr), "r"(__float_as_uint(v)), "r"(tag) : "memory");
+        asm volatile("st.relaxed.cluster.shared::cluster.b64 [%0], %1;" ::"r"(raddr), "l"(tw_pack(__float_as_uint(v), tag)) : "memory");
     }
     static __device__ __forceinline__ bool ld_sm(const W *p, uint32_t tag, float &v)
     {
-        uint32_t a, b;
-        asm volatile("ld.relaxed.cluster.shared::cta.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
-        v = __uint_as_float(a);
-        return b == tag;
+        uint64_t w;
+        asm volatile("ld.relaxed.cluster.shared::cta.b64 %0, [%1];" : "=l"(w) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
+        v = __uint_as_float((uint32_t)w);
+        return (uint32_t)(w >> 32) == tag;
     }
 };
 template <> struct Tagged<double> {
-    typedef uint4 W;
+    typedef ulonglong2 W;
     static __device__ __forceinline__ void st(W *p, double v, uint32_t tag)
     {
-        const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
-        asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag) : "memory");
+        const uint64_t lo = tw_pack((uint32_t)__double2loint(v), tag), hi = tw_pack((uint32_t)__double2hiint(v), tag);
+        asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(lo), "l"(hi) : "memory");
     }
     static __device__ __forceinline__ bool ld(const W *p, uint32_t tag, double &v)
     {
-        uint32_t a, b, c, d;
-        asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(p) : "memory");
-        v = __hiloint2double((int)c, (int)a);
-        return b == tag && d == tag;
+        uint64_t lo, hi;
+        asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(lo), "=l"(hi) : "l"(p) : "memory");
+        v = __hiloint2double((int)(uint32_t)hi, (int)(uint32_t)lo);
+        return (uint32_t)(lo >> 32) == tag && (uint32_t)(hi >> 32) == tag;
     }
     static __device__ __forceinline__ void st_cl(uint32_t raddr, double v, uint32_t tag)
     {
-        const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
-        asm volatile("st.relaxed.cluster.shared::cluster.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(raddr), "r"(lo), "r"(tag), "r"(hi), "r"(tag) : "memory");
+        const uint64_t lo = tw_pack((uint32_t)__double2loint(v), tag), hi = tw_pack((uint32_t)__double2hiint(v), tag);
+        asm volatile("st.relaxed.cluster.shared::cluster.v2.b64 [%0], {%1, %2};" ::"r"(raddr), "l"(lo), "l"(hi) : "memory");
     }
     static __device__ __forceinline__ bool ld_sm(const W *p, uint32_t tag, double &v)
     {
-        uint32_t a, b, c, d;
-        asm volatile("ld.relaxed.cluster.shared::cta.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
-        v = __hiloint2double((int)c, (int)a);
-        return b == tag && d == tag;
+        uint64_t lo, hi;
+        asm volatile("ld.relaxed.cluster.shared::cta.v2.b64 {%0, %1}, [%2];" : "=l"(lo), "=l"(hi) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
+        v = __hiloint2double((int)(uint32_t)hi, (int)(uint32_t)lo);
+        return (uint32_t)(lo >> 32) == tag && (uint32_t)(hi >> 32) == tag;
     }
 };
 
@@ -143,15 +149,6 @@ struct OCfg {
 };
 
 template <typename T> struct OState { T z, v, th, be, la, d, de; };
-
-// Developer aid (off by default): -DPIMPC_COOP_PROF accumulates clock64() per phase in CTA 0 and prints the means.
-#ifdef PIMPC_COOP_PROF
-#define PROF_DECL long long prof_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, prof_last = clock64();
-#define PROF_MARK(i) { const long long t_ = clock64(); prof_t[i] += t_ - prof_last; prof_last = t_; }
-#else
-#define PROF_DECL
-#define PROF_MARK(i)
-#endif
 
 // CL: the grid is ONE thread-block cluster (<= 16 CTAs) and the tagged words travel through distributed shared memory
 // (a remote store lands in ~200 cycles) instead of L2 (850-1000 cycles per hop, 2400+ for an all-to-all of 64 CTAs).
@@ -254,7 +251,6 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     bool done = false;
     __syncthreads();
     if (CL) cluster_sync_all();                  // every CTA of the cluster has zeroed its inbound words
-    PROF_DECL
 
     // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.  par = it & 1.
     auto iteration = [&](OState<T> (&cur)[SPG], OState<T> (&prv)[SPG], const int it, const int par) -> bool {
@@ -278,9 +274,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             if (has_e && exist[s]) { ev[s] = blkp[s][OE + li]; w -= ev[s]; }
             if (exist[s]) { blkp[s][OW + li] = w; blkp[s][OD + li] = dv[s]; }
         }
-        PROF_MARK(0)
         __syncthreads();
-        PROF_MARK(1)
         // ---- B: step 1: g = Abar_{k+1}^T w_{k+1}, h_k; rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat] ----
 #pragma unroll
         for (int s = 0; s < SPG; ++s) {
@@ -341,9 +335,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 if (ulane) blkp[s][ODU + li - NX] = du[s];
             }
         }
-        PROF_MARK(2)
         __syncthreads();
-        PROF_MARK(3)
         // ---- D: steps 2-4 of the real stages ----
         T acc = (T)0;
 #pragma unroll
@@ -414,9 +406,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 #pragma unroll
         for (int o = 16; o >= LPS; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
         if (lane == 0 && !comm) red[warp] = sum;
-        PROF_MARK(4)
         __syncthreads();
-        PROF_MARK(5)
         if (comm) {
             sum = lane < ncw ? red[lane] : 0.0;
 #pragma unroll
@@ -485,9 +475,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 }
             }
         }
-        PROF_MARK(6)
         __syncthreads();
-        PROF_MARK(7)
         // ---- steps 5-7; every thread of every CTA decides from the same bits ----
         const double c = red[32 + par], c_prev = red[32 + (par ^ 1)];
         it_done = it + 1;
@@ -513,12 +501,6 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         if (iteration(sb, sa, it + 1, 1)) { in_b = false; break; }
         in_b = false;
     }
-#ifdef PIMPC_COOP_PROF
-    if ((cta == 0 || cta == G / 2) && (tid == 0 || tid == ncw * 32) && it_done > 0)
-        printf("coop prof cta %d tid %d: A %lld | B1 %lld | BC %lld | B2 %lld | D %lld | B3 %lld | xchg %lld | B4 %lld cycles/it\n", cta, tid,
-               prof_t[0] / it_done, prof_t[1] / it_done, prof_t[2] / it_done, prof_t[3] / it_done, prof_t[4] / it_done,
-               prof_t[5] / it_done, prof_t[6] / it_done, prof_t[7] / it_done);
-#endif
     // ---- results: iterate -> S[i_cur], xbar and Delta u of the last iteration, control block ----
 #pragma unroll
     for (int s = 0; s < SPG; ++s) {
@@ -548,12 +530,6 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 
 struct CoopPlan { int grid, spg, threads, slots; size_t smem; int cluster; };
 
-int env_int_o(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    return v && *v ? atoi(v) : dflt;
-}
-
 // Horizons up to this length run as ONE cluster of 16 CTAs (B200, C3 generator, us per iteration, cluster vs 64 CTAs over
 // L2: fp32 N=100 1.24 / 2.34, 200 1.42 / 2.25, 400 1.83 / 2.58, 700 2.57 / 2.55; fp64 N=100 1.56 / 2.45, 200 1.91 / 2.57,
 // 400 2.75 / 2.70); beyond it the ranges per CTA get too long and more CTAs exchanging through L2 win.
@@ -566,17 +542,17 @@ bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
     const int gmax = std::min(h->sm_count, 32 * C::MAXJ);
     // ranges of >= 16 stages until 64 CTAs are busy, then as many CTAs as SMs (measured: the exchange grows with the grid)
     int grid = std::min(gmax, std::max((h->N + 15) / 16, std::min(h->N, 64)));
-    // short horizons: ONE cluster of <= 16 CTAs exchanging through distributed shared memory (PIMPC_COOP_CLUSTER = 0
-    // disables, = n forces n CTAs; default 16 while N <= CL_MAXN)
-    const int cl_env = env_int_o("PIMPC_COOP_CLUSTER", -1);
-    int cluster = cl_env >= 0 ? std::min(cl_env, C::CLMAX) : (h->N <= (sizeof(T) == 4 ? CL_MAXN_F32 : CL_MAXN_F64) ? C::CLMAX : 0);
+    // short horizons: ONE cluster of <= 16 CTAs exchanging through distributed shared memory (opts.tune.cluster = -1
+    // disables, = n forces n CTAs; automatic: 16 while N <= CL_MAXN)
+    const int cl_opt = h->tune.cluster;
+    int cluster = cl_opt != 0 ? std::min(std::max(cl_opt, 0), C::CLMAX) : (h->N <= (sizeof(T) == 4 ? CL_MAXN_F32 : CL_MAXN_F64) ? C::CLMAX : 0);
     if (cluster > 0) { cluster = std::min(cluster, h->N); grid = cluster; }
-    const int gforce = env_int_o("PIMPC_COOP_GRID", 0);        // test hook: fewer CTAs = longer ranges per CTA
+    const int gforce = h->tune.grid;                           // fewer CTAs = longer ranges per CTA
     if (gforce > 0) { grid = std::min(grid, gforce); if (cluster) cluster = grid; }
     const int L = (h->N + grid - 1) / grid;                    // longest range
     const int slots = L + 2, gpw = 32 / C::LPS;
     const int spg_max = sizeof(T) == 8 ? 1 : 2;
-    int spg = std::min(spg_max, std::max(1, env_int_o("PIMPC_COOP_SPG", 1)));   // test hook: stages per lane group
+    int spg = std::min(spg_max, std::max(1, h->tune.stages_per_group));         // stages per lane group
     while (spg <= spg_max && ((slots + spg - 1) / spg + gpw - 1) / gpw > 31) ++spg;
     if (spg > spg_max) { if (why) *why = "horizon too long for the register-resident iterates of the COOP engine"; return false; }
     const int ncw = ((slots + spg - 1) / spg + gpw - 1) / gpw;
@@ -620,11 +596,7 @@ int launch_coop(pimpc_s *h, int iters, double tol, const CoopPlan &pl)
     if (occ < 1) { h->errmsg = "COOP kernel does not fit on an SM"; return PIMPC_EINVAL; }
     const size_t pbytes = 2 * (size_t)(pl.grid + C::NREP) * C::PSTRIDE * sizeof(PW), hbytes = 2 * (size_t)pl.grid * C::HALO * sizeof(HW);
     const size_t need = pbytes + hbytes;
-    if (h->coop_bytes < need) {
-        if (h->coop_buf) { cudaFree(h->coop_buf); h->device_bytes -= h->coop_bytes; h->coop_buf = nullptr; h->coop_bytes = 0; }
-        if (cudaMalloc(&h->coop_buf, need) != cudaSuccess) { cudaGetLastError(); h->errmsg = "cudaMalloc (COOP exchange) failed"; return PIMPC_ENOMEM; }
-        h->coop_bytes = need; h->device_bytes += need;
-    }
+    { const int rc = pimpc_grow(h, &h->coop_buf, &h->coop_bytes, need); if (rc) return rc; }
     PIMPC_CUDA_TRY(h, cudaMemsetAsync(h->coop_buf, 0, need, h->stream));       // tag 0 = nothing published yet
     Prob<T> p = make_prob<T>(h, tol);
     PW *part = (PW *)h->coop_buf;

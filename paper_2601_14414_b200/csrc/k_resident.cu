@@ -15,8 +15,6 @@
 // c is reduced in a fixed order (xor butterflies; every warp repeats the second level), so every
 // thread takes the same accept/restart decision (steps 5-7) from bit-identical numbers.
 #include <algorithm>
-#include <cstdio>
-#include <cstdlib>
 
 #include "pimpc_internal.h"
 
@@ -99,15 +97,6 @@ struct RCfg {
         return ((NS + 2) * SS + KAPN) * sizeof(T) + 36 * sizeof(double);
     }
 };
-
-// Developer aid (off by default): -DPIMPC_RES_PROF accumulates clock64() per phase in CTA 0 and prints the means.
-#ifdef PIMPC_RES_PROF
-#define RPROF_DECL long long prof_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, prof_last = clock64();
-#define RPROF_MARK(i) { const long long t_ = clock64(); prof_t[i] += t_ - prof_last; prof_last = t_; }
-#else
-#define RPROF_DECL
-#define RPROF_MARK(i)
-#endif
 
 template <typename T, int R>
 struct RState { T z[R], v[R], th[R], be[R], la[R], d[R], de[R]; };
@@ -193,7 +182,6 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             sBlk[OX + tid] = tid < NX ? p.x0[(size_t)b * NX + tid] : (tid < NB ? p.uprev[(size_t)b * NU + (tid - NX)] : (T)0);
         if (tid == 0) { red[32] = p.c0; red[33] = p.c0; sCnt[0] = 0; }
 
-        RPROF_DECL
         T kap = (T)0;
         int jacc = 0, it_done = 0;
         bool done = false;
@@ -224,9 +212,7 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             }
             st_rows<T, R>(own + OW, wv);
             st_rows<T, R>(own + OD, dv);
-            RPROF_MARK(0)
             __syncthreads();
-            RPROF_MARK(1)
             // step 1: g = Abar_{k+1}^T w_{k+1}, rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat]
             T g[R][2], rd[R][2];
 #pragma unroll
@@ -260,7 +246,6 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 if (!isx[r]) own[ORH - NX + r] = rr;
             }
             st_rows<T, R>(own + OH, hv);
-            RPROF_MARK(2)
             __syncwarp();
             T x[R][2], du2[R][2], du[R];
 #pragma unroll
@@ -293,9 +278,7 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 if (!isx[r]) own[ODU - NX + r] = du[r];
             }
             st_rows<T, R>(own + OX, xs);
-            RPROF_MARK(3)
             __syncthreads();
-            RPROF_MARK(4)
             // steps 2-4
             T dot[R][2], av2[R][2], avx[R];
 #pragma unroll
@@ -354,10 +337,8 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             double s = (double)acc;
 #pragma unroll
             for (int o = 16; o >= LPS; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-            RPROF_MARK(5)
             if (lane == 0) red[warp] = s;
             __syncthreads();
-            RPROF_MARK(6)
             const double c_prev = red[32 + (par ^ 1)];
             // every warp repeats the second level (butterfly over the warp partials): same bits everywhere.  A shuffle-free
             // tree of 16 broadcast loads + DADDs per lane was measured 4 % slower on C4 (B200).
@@ -374,7 +355,6 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
                 if (!accept && !stop) ++sCnt[0];
                 if (hc && it < p.hist_cap) { hc[it] = c; ha[it] = (unsigned char)accept; }
             }
-            RPROF_MARK(7)
             if (stop) { done = true; return true; }
             if (accept) {
                 kap = jacc < C::KAPN ? sKap[jacc] : (T)kappa_tab[jacc];
@@ -394,12 +374,6 @@ k_resident(const Prob<T> p, const double *__restrict__ alpha_tab, const double *
             if (iteration(sb, sa, it + 1, 1)) { in_b = false; break; }
             in_b = false;
         }
-#ifdef PIMPC_RES_PROF
-        if (b == 0 && (tid == 0 || tid == 32 * (nwarps - 1)) && it_done > 0)
-            printf("res prof tid %d: A %lld | B1 %lld | B %lld | C %lld | B2 %lld | D+shfl %lld | B3 %lld | decide %lld cycles/it\n", tid,
-                   prof_t[0] / it_done, prof_t[1] / it_done, prof_t[2] / it_done, prof_t[3] / it_done, prof_t[4] / it_done,
-                   prof_t[5] / it_done, prof_t[6] / it_done, prof_t[7] / it_done);
-#endif
         if (in_b) sa = sb;                       // register moves; a reference select would force local memory
         const RState<T, R> &fin = sa;
 
@@ -475,11 +449,11 @@ int ensure_alpha_table(pimpc_s *h, int iters)
 {
     int launches = 0;
     if (h->tab_cap < iters + 2) {
-        if (h->alpha_tab) { cudaFree(h->alpha_tab); cudaFree(h->kappa_tab); h->alpha_tab = h->kappa_tab = nullptr; }
         const int cap = std::max(iters + 2, 1024);
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->alpha_tab, cap * sizeof(double)));
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->kappa_tab, cap * sizeof(double)));
-        h->device_bytes += 2 * (size_t)cap * sizeof(double);
+        size_t ca = (size_t)h->tab_cap * sizeof(double), ck = ca;
+        int rc = pimpc_grow(h, (void **)&h->alpha_tab, &ca, cap * sizeof(double));
+        if (!rc) rc = pimpc_grow(h, (void **)&h->kappa_tab, &ck, cap * sizeof(double));
+        if (rc) { h->tab_cap = 0; return rc; }
         k_alpha_table<<<1, 32, 0, h->stream>>>(h->alpha_tab, h->kappa_tab, cap);
         PIMPC_CUDA_TRY(h, cudaGetLastError());
         h->tab_cap = cap;
@@ -496,8 +470,7 @@ int run_resident(pimpc_s *h, int iters, double tol)
     if (launches < 0) return launches;
     int nwarps = (h->N + pl.spw - 1) / pl.spw;
     int n;
-    const char *rv = getenv("PIMPC_RESIDENT_R");         // tuning hook: 1 = one row per lane (16 lanes per stage)
-    if (h->dtype == PIMPC_F32 && h->nx == 12 && !(rv && atoi(rv) == 1) && h->N <= 56) {
+    if (h->dtype == PIMPC_F32 && h->nx == 12 && h->tune.rows_per_lane != 1 && h->N <= 56) {   // tune: 1 = one row per lane (16 lanes per stage)
         // two rows per lane, 8 lanes per stage: half the broadcast loads per FMA.  C4 on B200: 8.23 ms, against 9.11 ms
         // with one row per lane and 8.94 ms with four
         nwarps = (h->N + 3) / 4;

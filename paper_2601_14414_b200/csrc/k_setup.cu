@@ -2,6 +2,8 @@
 // bookkeeping kernels (begin / gather / state I/O).  One CTA per (instance, stage); the SPD
 // matrix lives in shared memory in double precision whatever the handle's dtype and is inverted
 // in place by Gauss-Jordan exchange steps without pivoting (safe for SPD matrices).
+#include <algorithm>
+
 #include "pimpc_internal.h"
 
 namespace {
@@ -32,13 +34,15 @@ __device__ bool gj_invert(double *S, double *colb, double *rowb, int n)
     return ok;
 }
 
+// list != null: only the cache entries of the listed flattened stage indices (b * N + k) are recomputed.
 template <typename T>
-__global__ void __launch_bounds__(256) k_setup(Prob<T> p)
+__global__ void __launch_bounds__(256) k_setup(Prob<T> p, const int *__restrict__ list)
 {
     extern __shared__ double sm[];
     const int nx = p.nx, nu = p.nu, nb = p.nb, N = p.N;
     double *S = sm, *colb = S + nb * nb, *rowb = colb + nb;
-    const int k = blockIdx.x, b = blockIdx.y;
+    const int sflat = list ? list[blockIdx.x] : (int)blockIdx.x;
+    const int b = sflat / N, k = sflat - b * N;
     const int tid = threadIdx.x, nt = blockDim.x;
     const bool last = (k == N - 1);
     const T *A1 = p.A + ((size_t)b * N + (last ? k : k + 1)) * nx * nx;
@@ -146,16 +150,17 @@ __device__ __forceinline__ bool gj_rows(double (&S)[W], double *rowb, const int 
 }
 
 template <typename T, int NX, int NU>
-__global__ void __launch_bounds__(128) k_setup_small(Prob<T> p)
+__global__ void __launch_bounds__(128) k_setup_small(Prob<T> p, const int *__restrict__ list, const long long nlist)
 {
     constexpr int NB = NX + NU, LPS = pow2ceil_k(NB), SPW = 32 / LPS, GPB = 4 * SPW, TS = LPS + 1;
     constexpr int GSZ = (NX * LPS > LPS * TS ? NX * LPS : LPS * TS) + LPS;
     static_assert(GSZ % 2 == 0 && LPS % 2 == 0, "16-byte alignment of the per-group buffers");
     __shared__ __align__(16) double sm[GPB * GSZ];
     const int tid = threadIdx.x, g = tid / LPS, li = tid % LPS, N = p.N;
-    const long long nst = (long long)p.batch * N, sraw = (long long)blockIdx.x * GPB + g;
+    const long long nst = list ? nlist : (long long)p.batch * N, sraw = (long long)blockIdx.x * GPB + g;
     const bool act = sraw < nst;
-    const long long sidx = act ? sraw : nst - 1;               // idle groups repeat the last stage and do not store
+    const long long spos = act ? sraw : nst - 1;               // idle groups repeat the last stage and do not store
+    const long long sidx = list ? (long long)list[spos] : spos;
     const int b = (int)(sidx / N), k = (int)(sidx - (long long)b * N);
     double *buf = sm + g * GSZ, *rowb = buf + (GSZ - LPS);
     const bool last = (k == N - 1), rowok = li < NB;
@@ -262,7 +267,7 @@ __global__ void k_begin(Prob<T> p)
 }
 
 template <typename T>
-__global__ void k_gather(Prob<T> p, T *x, T *u, T *du, pimpc_result *res)
+__global__ void k_gather(Prob<T> p, T *x, T *u, T *du)
 {
     const int b = blockIdx.y;
     const InstCtl c = p.ctl[b];
@@ -278,12 +283,65 @@ __global__ void k_gather(Prob<T> p, T *x, T *u, T *du, pimpc_result *res)
             du[((size_t)b * p.N + k) * p.nu + (i - p.nb)] = p.DU[((size_t)b * p.N + k) * p.nu + (i - p.nb)];
         }
     }
-    if (res && blockIdx.x == 0 && threadIdx.x == 0) {
-        pimpc_result r;
-        r.c = c.c_last; r.alpha = c.alpha; r.iters = c.iters; r.restarts = c.restarts;
-        r.converged = c.done; r.pad_ = 0;
-        res[b] = r;
+}
+
+// Result record of one instance per CTA.  r_prim2 = rho ||F p + G q - h||^2 of the returned iterate, from the definition
+// of the three (four with the Delta-u box) consensus constraints of Problem (11) ((14a), (15c)):
+//   xbar_{k+1} - z_{k+1},   Bbar_k Delta u_k - v_k,   z_{k+1} - Abar_k xbar_k - v_k - ebar_k   [, Delta u_k - d_k]
+// accumulated in double in a fixed order (thread-strided, then a fixed tree), r_dual2 = c - r_prim2.
+template <typename T>
+__global__ void __launch_bounds__(128) k_rprim(Prob<T> p, double *__restrict__ part, const int chunk)
+{
+    __shared__ double red[128];
+    const int b = blockIdx.y, nx = p.nx, nu = p.nu, nb = p.nb, N = p.N;
+    const InstCtl c = p.ctl[b];
+    const T *S = p.S + (size_t)c.i_cur * p.buf_stride;
+    double acc = 0.0;
+    const int i0 = blockIdx.x * chunk, i1 = min(N * nb, i0 + chunk);
+    for (int idx = i0 + threadIdx.x; idx < i1; idx += blockDim.x) {
+        const int k = idx / nb, i = idx - k * nb;
+        const size_t sk = (size_t)b * N + k;
+        const T *rec = S + p.st(b, k);
+        const double z = (double)rec[p.oZ() + i], v = (double)rec[p.oV() + i], xk1 = (double)p.X[sk * nb + i];
+        const T *du = p.DU + sk * nu;
+        double bdu, axk;                                       // (Bbar_k Delta u_k)_i, (Abar_k xbar_k + ebar_k)_i
+        if (i < nx) {
+            const T *Ak = p.A + sk * nx * nx + (size_t)i * nx, *Bk = p.B + sk * nx * nu + (size_t)i * nu;
+            bdu = 0.0; axk = p.e ? (double)p.e[sk * nx + i] : 0.0;
+            for (int j = 0; j < nu; ++j) bdu += (double)Bk[j] * (double)du[j];
+            for (int j = 0; j < nx; ++j) axk += (double)Ak[j] * (double)(k == 0 ? p.x0[(size_t)b * nx + j] : p.X[(sk - 1) * nb + j]);
+            for (int j = 0; j < nu; ++j) axk += (double)Bk[j] * (double)(k == 0 ? p.uprev[(size_t)b * nu + j] : p.X[(sk - 1) * nb + nx + j]);
+        } else {
+            bdu = (double)du[i - nx];
+            axk = (double)(k == 0 ? p.uprev[(size_t)b * nu + (i - nx)] : p.X[(sk - 1) * nb + i]);
+        }
+        const double r1 = xk1 - z, r2 = bdu - v, r3 = z - axk - v;
+        acc += r1 * r1 + r2 * r2 + r3 * r3;
+        if (p.has_du && i >= nx) { const double r4 = (double)du[i - nx] - (double)rec[p.oD() + (i - nx)]; acc += r4 * r4; }
     }
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[(size_t)b * gridDim.x + blockIdx.x] = red[0];
+}
+
+__global__ void k_result(const InstCtl *__restrict__ ctl, const double *__restrict__ part, const int nch, const int batch,
+                         const double rho, pimpc_result *res)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    const InstCtl c = ctl[b];
+    double s = 0.0;
+    for (int q = 0; q < nch; ++q) s += part[(size_t)b * nch + q];
+    pimpc_result r;
+    r.c = c.c_last; r.alpha = c.alpha; r.iters = c.iters; r.restarts = c.restarts;
+    r.converged = c.done; r.pad_ = 0;
+    r.r_prim2 = c.iters > 0 ? rho * s : 0.0;
+    r.r_dual2 = c.iters > 0 ? c.c_last - r.r_prim2 : 0.0;
+    res[b] = r;
 }
 
 // which: PIMPC_X.. ; set = 0: state -> dense buffer, 1: dense buffer -> state (current iterate).
@@ -381,32 +439,36 @@ template Prob<float> make_prob<float>(pimpc_s *, double);
 template Prob<double> make_prob<double>(pimpc_s *, double);
 
 template <typename T, int NX, int NU>
-static int setup_small_t(pimpc_s *h)
+static int setup_small_t(pimpc_s *h, const int *list, int nlist)
 {
     Prob<T> p = make_prob<T>(h, 0.0);
     constexpr int GPB = 4 * (32 / pow2ceil_k(NX + NU));
-    const long long nst = (long long)h->batch * h->N;
-    k_setup_small<T, NX, NU><<<(unsigned)((nst + GPB - 1) / GPB), 128, 0, h->stream>>>(p);
+    const long long nst = list ? nlist : (long long)h->batch * h->N;
+    k_setup_small<T, NX, NU><<<(unsigned)((nst + GPB - 1) / GPB), 128, 0, h->stream>>>(p, list, nst);
     PIMPC_CUDA_TRY(h, cudaGetLastError());
     return 1;
 }
 
 template <typename T>
-static int setup_t(pimpc_s *h)
+static int setup_t(pimpc_s *h, const int *list, int nlist)
 {
-    if (h->nx == 12 && h->nu == 4) return setup_small_t<T, 12, 4>(h);
-    if (h->nx == 4 && h->nu == 2) return setup_small_t<T, 4, 2>(h);
+    if (h->nx == 12 && h->nu == 4) return setup_small_t<T, 12, 4>(h, list, nlist);
+    if (h->nx == 4 && h->nu == 2) return setup_small_t<T, 4, 2>(h, list, nlist);
     Prob<T> p = make_prob<T>(h, 0.0);
     const size_t smem = ((size_t)h->nb * h->nb + 2 * h->nb) * sizeof(double);
     if (smem > 48 * 1024)
         PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(k_setup<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int threads = h->nb * h->nb >= 1024 ? 256 : 128;
-    k_setup<T><<<dim3(h->N, h->batch), threads, smem, h->stream>>>(p);
+    const long long nst = list ? nlist : (long long)h->batch * h->N;
+    k_setup<T><<<(unsigned)nst, threads, smem, h->stream>>>(p, list);
     PIMPC_CUDA_TRY(h, cudaGetLastError());
     return 1;
 }
 
-int launch_setup(pimpc_s *h) { return h->dtype == PIMPC_F64 ? setup_t<double>(h) : setup_t<float>(h); }
+int launch_setup(pimpc_s *h, const int *list_dev, int nlist)
+{
+    return h->dtype == PIMPC_F64 ? setup_t<double>(h, list_dev, nlist) : setup_t<float>(h, list_dev, nlist);
+}
 
 int launch_begin(pimpc_s *h)
 {
@@ -421,12 +483,26 @@ int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res)
 {
     const int work = h->N * (h->nb + h->nu);
     const int th = 256, bl = min(64, (work + th - 1) / th);
-    if (h->dtype == PIMPC_F64)
-        k_gather<double><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<double>(h, 0.0), (double *)x, (double *)u, (double *)du, res);
-    else
-        k_gather<float><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<float>(h, 0.0), (float *)x, (float *)u, (float *)du, res);
+    int n = 0;
+    if (x || u || du) {
+        if (h->dtype == PIMPC_F64)
+            k_gather<double><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<double>(h, 0.0), (double *)x, (double *)u, (double *)du);
+        else
+            k_gather<float><<<dim3(bl, h->batch), th, 0, h->stream>>>(make_prob<float>(h, 0.0), (float *)x, (float *)u, (float *)du);
+        ++n;
+    }
+    if (res) {
+        const int rows = h->N * h->nb;
+        const int nch = std::max(1, std::min(64, rows / 2048)), chunk = (rows + nch - 1) / nch;
+        const int rc = pimpc_grow(h, (void **)&h->res_part, &h->res_part_cap, (size_t)h->batch * nch * sizeof(double));
+        if (rc) return rc;
+        if (h->dtype == PIMPC_F64) k_rprim<double><<<dim3(nch, h->batch), 128, 0, h->stream>>>(make_prob<double>(h, 0.0), h->res_part, chunk);
+        else k_rprim<float><<<dim3(nch, h->batch), 128, 0, h->stream>>>(make_prob<float>(h, 0.0), h->res_part, chunk);
+        k_result<<<(h->batch + 127) / 128, 128, 0, h->stream>>>(h->ctl, h->res_part, nch, h->batch, h->rho, res);
+        n += 2;
+    }
     PIMPC_CUDA_TRY(h, cudaGetLastError());
-    return 1;
+    return n;
 }
 
 int launch_state_io(pimpc_s *h, int which, void *buf, int set)

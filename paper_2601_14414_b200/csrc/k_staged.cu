@@ -245,17 +245,14 @@ int run_staged_t(pimpc_s *h, int iters, double tol)
     const int threads = ((spb * nb + 31) / 32) * 32;   // whole warps (idle lanes are masked by ks >= spb)
     const int gx = (h->N + spb - 1) / spb;
     const size_t nst = (size_t)h->batch * h->N;
-    if (!h->hat) {
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->hat, nst * h->rec * h->esz));
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->W, nst * nb * h->esz));
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->G, nst * nb * h->esz));
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->rhs, nst * h->nu * h->esz));
-        h->device_bytes += nst * (h->rec + 2 * nb + h->nu) * h->esz;
-    }
-    if (gx > h->nparts_cap) {
-        if (h->partial) cudaFree(h->partial);
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->partial, (size_t)h->batch * gx * sizeof(double)));
-        h->nparts_cap = gx;
+    {
+        size_t c0 = h->hat ? ~(size_t)0 : 0, c1 = c0, c2 = c0, c3 = c0;            // allocated once per handle (sizes are fixed)
+        int rc = pimpc_grow(h, &h->hat, &c0, nst * h->rec * h->esz);
+        if (!rc) rc = pimpc_grow(h, &h->W, &c1, nst * nb * h->esz);
+        if (!rc) rc = pimpc_grow(h, &h->G, &c2, nst * nb * h->esz);
+        if (!rc) rc = pimpc_grow(h, &h->rhs, &c3, nst * h->nu * h->esz);
+        if (!rc) rc = pimpc_grow(h, (void **)&h->partial, &h->partial_cap, (size_t)h->batch * gx * sizeof(double));
+        if (rc) return rc;
     }
     Prob<T> p = make_prob<T>(h, tol);
     p.nparts = gx;

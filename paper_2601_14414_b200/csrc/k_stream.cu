@@ -516,12 +516,6 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
     }
 }
 
-int env_int(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    return v && *v ? atoi(v) : dflt;
-}
-
 struct StreamPlan { int grid, nslot; size_t smem; };
 
 template <typename T, int NX, int NU>
@@ -532,9 +526,9 @@ int plan_stream(pimpc_s *h, StreamPlan *pl)
     const size_t fixed = ((sizeof(StreamSmem) + 127) / 128) * 128 + (size_t)C::V_END * sizeof(T);
     const size_t slot = (size_t)C::SLOT * sizeof(T);
     // CTAs per SM: enough bytes in flight per SM to cover the HBM latency (>= 2 slots per CTA), several
-    // CTAs so that one CTA's step barriers overlap another's math; tuning overrides via the environment.
+    // CTAs so that one CTA's step barriers overlap another's math; opts.tune overrides.
     const size_t per_sm = 227 * 1024;
-    int want = env_int("PIMPC_STREAM_CTAS_PER_SM", 0);
+    int want = h->tune.ctas_per_sm;
     if (want <= 0) want = slot > 32 * 1024 ? 2 : (slot > 8 * 1024 ? 4 : 6);   // C5 fp32: 4 CTAs per SM 0.73 ms/it, 3: 0.82, 2: 1.04
     int nslot = 0, per = want;
     for (; per >= 1; --per) {
@@ -543,7 +537,7 @@ int plan_stream(pimpc_s *h, StreamPlan *pl)
         nslot = (int)std::min<size_t>((budget - fixed) / slot, StreamSmem::MAXSLOT);
         if (nslot >= 2 || per == 1) break;
     }
-    const int force = env_int("PIMPC_STREAM_NSLOT", 0);
+    const int force = h->tune.ring_slots;
     if (force > 0) nslot = std::min(force, nslot);
     if (nslot < 1) { h->errmsg = "STREAM: a ring slot does not fit in shared memory"; return PIMPC_EINVAL; }
     const size_t smem = fixed + (size_t)nslot * slot;
@@ -554,7 +548,7 @@ int plan_stream(pimpc_s *h, StreamPlan *pl)
     occ = std::min(occ, per);
     const long long S_tot = (long long)h->batch * (h->N + 1);
     long long grid = std::min<long long>(S_tot, (long long)h->sm_count * occ);
-    const int gforce = env_int("PIMPC_STREAM_GRID", 0);       // test hook: fewer CTAs = longer ranges per CTA
+    const int gforce = h->tune.grid;                          // fewer CTAs = longer ranges per CTA
     if (gforce > 0) grid = std::min<long long>(grid, gforce);
     // a CTA's range may touch at most MAXI instances
     while (grid > 1 && (S_tot / grid + 1) / (h->N + 1) + 2 > C::MAXI) grid /= 2;   // never true for the shapes AUTO sends here
@@ -573,18 +567,13 @@ int run_stream_t(pimpc_s *h, int iters, double tol)
     int launches = 0;
     const size_t nblob = (size_t)h->batch * (h->N + 1);
     const size_t bbytes = nblob * C::BLOB * sizeof(T);
-    if (!h->blob || h->blob_bytes != bbytes) {
-        if (h->blob) { cudaFree(h->blob); h->device_bytes -= h->blob_bytes; h->blob = nullptr; }
-        if (cudaMalloc(&h->blob, bbytes) != cudaSuccess) { cudaGetLastError(); h->errmsg = "cudaMalloc (stage blobs) failed"; return PIMPC_ENOMEM; }
-        h->blob_bytes = bbytes; h->device_bytes += bbytes; h->blob_dirty = true;
+    if (!h->blob || h->blob_bytes < bbytes) {
+        rc = pimpc_grow(h, &h->blob, &h->blob_bytes, bbytes); if (rc) return rc;
+        h->blob_dirty = true;
     }
     int span = (pl.grid + h->batch - 1) / h->batch + 2;        // CTAs whose ranges can touch one instance
     const size_t pneed = 2 * (size_t)h->batch * span;
-    if (h->spartial_cap < pneed) {
-        if (h->spartial) cudaFree(h->spartial);
-        PIMPC_CUDA_TRY(h, cudaMalloc(&h->spartial, pneed * sizeof(double)));
-        h->spartial_cap = pneed;
-    }
+    rc = pimpc_grow(h, (void **)&h->spartial, &h->spartial_cap, pneed * sizeof(double)); if (rc) return rc;
     Prob<T> p = make_prob<T>(h, tol);
     if (h->blob_dirty) {
         k_pack<T, NX, NU><<<dim3(h->N + 1, h->batch), 128, 0, h->stream>>>(p, (T *)h->blob);

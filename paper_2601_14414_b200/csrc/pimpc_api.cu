@@ -1,6 +1,8 @@
 // C ABI of libpimpc.so (include/pimpc.h): handle lifetime, host/device marshalling, engine choice.
 // Every arithmetic step of Algorithm 1 runs in the kernels of k_*.cu; nothing here computes.
+#include <algorithm>
 #include <cmath>
+#include <cstdint>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -25,13 +27,14 @@ bool is_device_ptr(const void *p)
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-// Copy `bytes` into device memory of the handle.  Host sources are consumed before returning.
+// Copy `bytes` into device memory of the handle, asynchronously on the handle's stream.  A pageable host source has
+// been staged by the CUDA runtime when cudaMemcpyAsync returns (it may be reused at once); a page-locked host source
+// or a device source is read when the stream reaches the copy (lifetime rule of include/pimpc.h).  No stream
+// synchronisation here: several uploads of one step queue back to back.
 int copy_in(pimpc_s *h, void *dst, const void *src, size_t bytes)
 {
     if (bytes == 0) return PIMPC_OK;
-    const bool dev = is_device_ptr(src);
-    PIMPC_CUDA_TRY(h, cudaMemcpyAsync(dst, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
-    if (!dev) PIMPC_CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    PIMPC_CUDA_TRY(h, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, h->stream));
     return PIMPC_OK;
 }
 
@@ -83,9 +86,14 @@ int fill_identity(pimpc_s *h, void *dst, int n)
     return PIMPC_OK;
 }
 
+// Device memory of the handle: carved from the caller's workspace (opts.workspace) while it lasts, else cudaMalloc.
 int dalloc(pimpc_s *h, void **p, size_t bytes)
 {
     if (bytes == 0) bytes = 16;
+    if (h->ws) {
+        const size_t need = (bytes + 255) / 256 * 256;
+        if (h->ws_used + need <= h->ws_bytes) { *p = h->ws + h->ws_used; h->ws_used += need; return PIMPC_OK; }
+    }
     cudaError_t e = cudaMalloc(p, bytes);
     if (e != cudaSuccess) {
         cudaGetLastError();
@@ -99,20 +107,15 @@ int dalloc(pimpc_s *h, void **p, size_t bytes)
 // whole device, on the result path).
 int staging(pimpc_s *h, size_t bytes, void **out)
 {
-    if (h->stage_bytes < bytes) {
-        if (h->stage_buf) { cudaStreamSynchronize(h->stream); cudaFree(h->stage_buf); h->device_bytes -= h->stage_bytes; h->stage_buf = nullptr; h->stage_bytes = 0; }
-        if (cudaMalloc(&h->stage_buf, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, PIMPC_ENOMEM, "cudaMalloc (staging) failed"); }
-        h->stage_bytes = bytes; h->device_bytes += bytes;
-    }
+    const int rc = pimpc_grow(h, &h->stage_buf, &h->stage_bytes, bytes);
     *out = h->stage_buf;
-    return PIMPC_OK;
+    return rc;
 }
 
 int rec_len(int nb, int nu) { return ((5 * nb + 2 * nu + 3) / 4) * 4; }
 
 struct Sizes {
     size_t A, B, e, x0, up, H, M, S, X, DU, cost, bnd, ctl;
-    size_t total() const { return A + B + x0 + up + H + M + S + X + DU + cost + bnd + ctl; }
 };
 
 Sizes sizes(int nx, int nu, int N, int batch, size_t esz)
@@ -136,6 +139,29 @@ int check_handle(pimpc_s *h)
     return PIMPC_OK;
 }
 
+// Every entry point that touches CUDA runs on the device the handle was created on, whatever the caller's current
+// device is (a single process may drive one handle per GPU), and restores the caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const pimpc_s *h)
+    {
+        if (!h) return;
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
+        if (prev != h->device) switched = cudaSetDevice(h->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+// pimpc_set_stage touched stage k of instance b: cache entries H_{k-1} (holds Abar_k) and M_k, H_k... of that instance
+void mark_stage_dirty(pimpc_s *h, int b, int k, bool hk_prev, bool mk)
+{
+    if (h->cache_dirty) return;
+    if (h->dirty_stages.size() > 4096) { h->cache_dirty = true; h->dirty_stages.clear(); return; }
+    if (hk_prev && k > 0) h->dirty_stages.push_back(b * h->N + k - 1);
+    if (mk) h->dirty_stages.push_back(b * h->N + k);
+}
+
 int deferred_error(pimpc_s *h)
 {
     int flag = 0;
@@ -152,6 +178,25 @@ int deferred_error(pimpc_s *h)
 
 } // namespace
 
+int pimpc_grow(pimpc_s *h, void **ptr, size_t *cap, size_t bytes)
+{
+    if (*ptr && *cap >= bytes) return PIMPC_OK;
+    if (*ptr) {
+        cudaStreamSynchronize(h->stream);        // the old buffer may still be in use by queued work
+        cudaFree(*ptr);
+        h->device_bytes -= *cap;
+        *ptr = nullptr; *cap = 0;
+    }
+    if (bytes == 0) bytes = 16;
+    if (cudaMalloc(ptr, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        *ptr = nullptr;
+        return fail(h, PIMPC_ENOMEM, "cudaMalloc (engine scratch) failed");
+    }
+    *cap = bytes; h->device_bytes += bytes;
+    return PIMPC_OK;
+}
+
 extern "C" {
 
 const char *pimpc_version(void) { return "pimpc-b200 0.1 (sm_100a)"; }
@@ -160,16 +205,29 @@ void pimpc_default_opts(pimpc_opts *o)
 {
     if (!o) return;
     o->dtype = PIMPC_F64; o->engine = PIMPC_ENGINE_AUTO; o->rho = 1.0; o->eta = 0.999; o->c0 = 1.0;
-    o->history = 0; o->stream = nullptr;
+    o->history = 0; o->stream = nullptr; o->workspace = nullptr; o->workspace_bytes = 0;
+    memset(&o->tune, 0, sizeof(o->tune));
+}
+
+// The allocations of pimpc_create, in order (dalloc rounds each to 256 bytes inside a workspace).
+static std::vector<size_t> create_allocs(int nx, int nu, int N, int batch, size_t esz, int history)
+{
+    const Sizes s = sizes(nx, nu, N, batch, esz);
+    const size_t nb = nx + nu, b = batch;
+    std::vector<size_t> v = {s.A, s.B, s.x0, s.up, s.H, s.M, s.S, s.X, s.DU,
+                             b * nx * nx * esz, b * nx * nx * esz, b * nu * nu * esz, b * nu * nu * esz, b * nb * esz,
+                             b * nb * esz, b * nb * esz, b * nu * esz, b * nu * esz, s.ctl, sizeof(int)};
+    if (history > 0) { v.push_back(b * history * sizeof(double)); v.push_back(b * (size_t)history); }
+    return v;
 }
 
 size_t pimpc_workspace_bytes(int nx, int nu, int N, int batch, const pimpc_opts *opts)
 {
-    if (nx <= 0 || nu <= 0 || N <= 0 || batch <= 0 || nx + nu > 128) return 0;
+    if (nx <= 0 || nu <= 0 || N <= 0 || batch <= 0 || nx + nu > PIMPC_MAX_NB || batch > 65535) return 0;
     const size_t esz = (opts && opts->dtype == PIMPC_F32) ? 4 : 8;
-    Sizes s = sizes(nx, nu, N, batch, esz);
-    size_t hist = (opts && opts->history > 0) ? (size_t)batch * opts->history * 9 : 0;
-    return s.total() + hist;
+    size_t tot = 0;
+    for (size_t a : create_allocs(nx, nu, N, batch, esz, opts ? opts->history : 0)) tot += (std::max<size_t>(a, 16) + 255) / 256 * 256;
+    return tot;
 }
 
 int pimpc_create(pimpc_t *out, int nx, int nu, int N, int batch, const pimpc_opts *opts)
@@ -183,7 +241,16 @@ int pimpc_create(pimpc_t *out, int nx, int nu, int N, int batch, const pimpc_opt
     if (o.eta < 0.0) o.eta = 0.999;
     if (o.c0 == 0.0) o.c0 = 1.0;
     if (nx <= 0 || nu <= 0 || N <= 0 || batch <= 0) return fail(nullptr, PIMPC_EINVAL, "nx, nu, N, batch must be positive");
-    if (nx + nu > 128) return fail(nullptr, PIMPC_EINVAL, "nx + nu > 128 is not supported");
+    if (nx + nu > PIMPC_MAX_NB) return fail(nullptr, PIMPC_EINVAL, "nx + nu > 160 is not supported");
+    if (batch > 65535) return fail(nullptr, PIMPC_EINVAL, "batch > 65535 is not supported (one handle per 65535 instances)");
+    if (o.workspace) {
+        if (((uintptr_t)o.workspace & 255) || !is_device_ptr(o.workspace)) return fail(nullptr, PIMPC_EINVAL, "workspace must be 256-byte aligned device memory");
+        if (o.workspace_bytes < pimpc_workspace_bytes(nx, nu, N, batch, &o)) return fail(nullptr, PIMPC_EINVAL, "workspace smaller than pimpc_workspace_bytes()");
+    }
+    const pimpc_tune &tu = o.tune;
+    if (tu.grid < 0 || tu.ctas_per_sm < 0 || tu.ring_slots < 0 || tu.stages_per_group < 0 || tu.stages_per_group > 2 ||
+        tu.cluster < -1 || tu.cluster > 16 || tu.rows_per_lane < 0 || tu.rows_per_lane > 2 || tu.lookahead < -1 || tu.lookahead > 1)
+        return fail(nullptr, PIMPC_EINVAL, "bad opts.tune");
     if (!(o.rho > 0.0) || !std::isfinite(o.rho)) return fail(nullptr, PIMPC_EINVAL, "rho must be positive");
     if (o.dtype != PIMPC_F64 && o.dtype != PIMPC_F32) return fail(nullptr, PIMPC_EINVAL, "bad dtype");
     if (o.engine < PIMPC_ENGINE_AUTO || o.engine > PIMPC_ENGINE_COOP) return fail(nullptr, PIMPC_EINVAL, "bad engine");
@@ -201,6 +268,8 @@ int pimpc_create(pimpc_t *out, int nx, int nu, int N, int batch, const pimpc_opt
     h->dtype = o.dtype; h->esz = o.dtype == PIMPC_F64 ? 8 : 4;
     h->engine_req = o.engine; h->rho = o.rho; h->eta = o.eta; h->c0 = o.c0; h->hist_cap = o.history;
     h->stream = (cudaStream_t)o.stream;
+    h->tune = o.tune;
+    h->ws = (unsigned char *)o.workspace; h->ws_bytes = o.workspace ? o.workspace_bytes : 0;
     cudaGetDevice(&h->device);
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, h->device) != cudaSuccess) { delete h; return fail(nullptr, PIMPC_ECUDA, "cudaGetDeviceProperties failed"); }
@@ -249,11 +318,14 @@ int pimpc_create(pimpc_t *out, int nx, int nu, int N, int batch, const pimpc_opt
 int pimpc_destroy(pimpc_t h)
 {
     if (!h) return PIMPC_OK;
+    DeviceGuard guard(h);
     if (!h->poisoned) cudaStreamSynchronize(h->stream);
     void *ptrs[] = {h->A, h->B, h->e, h->x0, h->uprev, h->Q, h->R, h->P, h->Wdu, h->qbar, h->lo, h->hi, h->dlo, h->dhi,
                     h->H, h->M, h->S, h->X, h->DU, h->ctl, h->partial, h->hist_c, h->hist_a, h->err,
-                    h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab, h->spartial, h->coop_buf, h->stage_buf};
-    for (void *p : ptrs) if (p) cudaFree(p);
+                    h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab, h->spartial, h->coop_buf, h->stage_buf,
+                    h->dirty_dev, h->res_part};
+    for (void *p : ptrs)                         // memory carved from the caller's workspace is the caller's
+        if (p && !(h->ws && (unsigned char *)p >= h->ws && (unsigned char *)p < h->ws + h->ws_bytes)) cudaFree(p);
     for (auto &e : h->ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();
     delete h;
@@ -266,10 +338,12 @@ int pimpc_set_stage(pimpc_t h, int b, int k, const void *A_k, const void *B_k, c
     int rc = check_handle(h);
     if (rc) return rc;
     if (b < 0 || b >= h->batch || k < 0 || k >= h->N) return fail(h, PIMPC_EINVAL, "instance or stage index out of range");
+    DeviceGuard guard(h);
     const size_t sk = (size_t)b * h->N + k, esz = h->esz;
     const int nx = h->nx, nu = h->nu, nb = h->nb;
-    if (A_k) { rc = copy_in(h, (char *)h->A + sk * nx * nx * esz, A_k, (size_t)nx * nx * esz); if (rc) return rc; h->cache_dirty = true; }
-    if (B_k) { rc = copy_in(h, (char *)h->B + sk * nx * nu * esz, B_k, (size_t)nx * nu * esz); if (rc) return rc; h->cache_dirty = true; }
+    // H_{k-1} holds Abar_k = [A_k B_k; 0 I], M_k holds B_k: only those cache entries are recomputed
+    if (A_k) { rc = copy_in(h, (char *)h->A + sk * nx * nx * esz, A_k, (size_t)nx * nx * esz); if (rc) return rc; mark_stage_dirty(h, b, k, true, false); h->blob_dirty = true; }
+    if (B_k) { rc = copy_in(h, (char *)h->B + sk * nx * nu * esz, B_k, (size_t)nx * nu * esz); if (rc) return rc; mark_stage_dirty(h, b, k, true, true); h->blob_dirty = true; }
     if (e_k) {
         if (!h->e) {
             rc = dalloc(h, &h->e, (size_t)h->batch * h->N * nx * esz); if (rc) return rc;
@@ -277,6 +351,7 @@ int pimpc_set_stage(pimpc_t h, int b, int k, const void *A_k, const void *B_k, c
         }
         rc = copy_in(h, (char *)h->e + sk * nx * esz, e_k, (size_t)nx * esz); if (rc) return rc;
         h->has_e = 1;
+        h->blob_dirty = true;                  // the STREAM engine reads e_k from its packed blobs
     }
     if (Q || R) {
         if (h->cost_per_instance) return fail(h, PIMPC_EINVAL, "per-instance cost is set; use pimpc_set_cost");
@@ -301,6 +376,7 @@ int pimpc_set_stages(pimpc_t h, const void *A, const void *B, const void *e)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     const size_t nst = (size_t)h->batch * h->N, esz = h->esz;
     if (A) { rc = copy_in(h, h->A, A, nst * h->nx * h->nx * esz); if (rc) return rc; h->cache_dirty = true; }
     if (B) { rc = copy_in(h, h->B, B, nst * h->nx * h->nu * esz); if (rc) return rc; h->cache_dirty = true; }
@@ -308,6 +384,7 @@ int pimpc_set_stages(pimpc_t h, const void *A, const void *B, const void *e)
         if (!h->e) { rc = dalloc(h, &h->e, nst * h->nx * esz); if (rc) return rc; }
         rc = copy_in(h, h->e, e, nst * h->nx * esz); if (rc) return rc;
         h->has_e = 1;
+        h->blob_dirty = true;                  // the STREAM engine reads e_k from its packed blobs
     }
     return PIMPC_OK;
 }
@@ -317,6 +394,7 @@ int pimpc_set_cost(pimpc_t h, const void *Q, const void *R, const void *P, const
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     if (!Q || !R) return fail(h, PIMPC_EINVAL, "Q and R are required");
     const size_t rep = per_instance ? h->batch : 1, esz = h->esz;
     const size_t nq = (size_t)h->nx * h->nx, nr = (size_t)h->nu * h->nu;
@@ -336,6 +414,7 @@ int pimpc_set_bounds(pimpc_t h, const void *lo, const void *hi, const void *du_l
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     if (!lo || !hi) return fail(h, PIMPC_EINVAL, "lo and hi are required (use +-inf for no bound)");
     if ((du_lo == nullptr) != (du_hi == nullptr)) return fail(h, PIMPC_EINVAL, "du_lo and du_hi must be given together");
     const size_t rep = per_instance ? h->batch : 1, esz = h->esz;
@@ -369,6 +448,7 @@ int pimpc_set_x0(pimpc_t h, const void *x0, const void *u_prev)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     if (!x0) return fail(h, PIMPC_EINVAL, "x0 is NULL");
     rc = copy_in(h, h->x0, x0, (size_t)h->batch * h->nx * h->esz); if (rc) return rc;
     if (u_prev) { rc = copy_in(h, h->uprev, u_prev, (size_t)h->batch * h->nu * h->esz); if (rc) return rc; }
@@ -380,15 +460,29 @@ int pimpc_solve(pimpc_t h, int max_iters, double tol)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     if (max_iters < 0) return fail(h, PIMPC_EINVAL, "max_iters < 0");
     if (h->hist_cap > 0 && max_iters > h->hist_cap) return fail(h, PIMPC_EINVAL, "max_iters exceeds opts.history");
     int launches = 0, n;
     PIMPC_CUDA_TRY(h, cudaEventRecord(h->ev[0], h->stream));
-    h->ev_setup = h->cache_dirty;
+    h->ev_setup = h->cache_dirty || !h->dirty_stages.empty();
     if (h->cache_dirty) {
-        n = launch_setup(h); if (n < 0) return n;
+        n = launch_setup(h, nullptr, 0); if (n < 0) return n;
         launches += n;
         h->cache_dirty = false;
+        h->dirty_stages.clear();
+        h->blob_dirty = true;
+    } else if (!h->dirty_stages.empty()) {
+        // pimpc_set_stage touched a few stages: only their cache entries are re-inverted
+        std::vector<int> &v = h->dirty_stages;
+        std::sort(v.begin(), v.end());
+        v.erase(std::unique(v.begin(), v.end()), v.end());
+        rc = pimpc_grow(h, (void **)&h->dirty_dev, &h->dirty_cap, v.size() * sizeof(int)); if (rc) return rc;
+        PIMPC_CUDA_TRY(h, cudaMemcpyAsync(h->dirty_dev, v.data(), v.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+        PIMPC_CUDA_TRY(h, cudaStreamSynchronize(h->stream));          // v is host memory that is cleared below
+        n = launch_setup(h, h->dirty_dev, (int)v.size()); if (n < 0) return n;
+        launches += n;
+        v.clear();
         h->blob_dirty = true;
     }
     n = launch_begin(h); if (n < 0) return n;
@@ -427,6 +521,7 @@ int pimpc_get(pimpc_t h, void *x, void *u, void *du, pimpc_result *res)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     const size_t nst = (size_t)h->batch * h->N, esz = h->esz;
     // gather into device staging when the destination is host memory
     void *dx = nullptr, *du_ = nullptr, *ddu = nullptr;
@@ -442,12 +537,13 @@ int pimpc_get(pimpc_t h, void *x, void *u, void *du, pimpc_result *res)
     du_ = hu ? sb + off : u; off += hu ? al(bu) : 0;
     ddu = hd ? sb + off : du; off += hd ? al(bu) : 0;
     dres = hr ? (pimpc_result *)(sb + off) : res;
-    if (!rc) rc = launch_gather(h, dx, du_, ddu, dres) < 0 ? PIMPC_ECUDA : PIMPC_OK;
+    int ng = 0;
+    if (!rc) { ng = launch_gather(h, dx, du_, ddu, dres); if (ng < 0) rc = PIMPC_ECUDA; }
     if (!rc && x && dx != x) rc = copy_out(h, x, dx, nst * h->nx * esz);
     if (!rc && u && du_ != u) rc = copy_out(h, u, du_, nst * h->nu * esz);
     if (!rc && du && ddu != du) rc = copy_out(h, du, ddu, nst * h->nu * esz);
     if (!rc && res && (void *)dres != (void *)res) rc = copy_out(h, res, dres, (size_t)h->batch * sizeof(pimpc_result));
-    h->info.total_launches += 1;
+    h->info.total_launches += ng > 0 ? ng : 0;
     return rc ? rc : deferred_error(h);        // synchronises
 }
 
@@ -464,6 +560,7 @@ int pimpc_get_state(pimpc_t h, int which, void *out)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     const int w = state_width(h, which);
     if (w < 0 || !out) return fail(h, PIMPC_EINVAL, "bad selector or NULL buffer");
     const size_t bytes = (size_t)h->batch * h->N * w * h->esz;
@@ -480,6 +577,7 @@ int pimpc_set_state(pimpc_t h, int which, const void *in)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     const int w = state_width(h, which);
     if (w < 0 || !in || which == PIMPC_X || which == PIMPC_DU) return fail(h, PIMPC_EINVAL, "bad selector (X, DU are outputs) or NULL buffer");
     const size_t bytes = (size_t)h->batch * h->N * w * h->esz;
@@ -498,6 +596,7 @@ int pimpc_get_history(pimpc_t h, double *c, unsigned char *accepted)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     if (h->hist_cap <= 0) return fail(h, PIMPC_EINVAL, "handle was created with history = 0");
     if (c) { rc = copy_out(h, c, h->hist_c, (size_t)h->batch * h->hist_cap * sizeof(double)); if (rc) return rc; }
     if (accepted) { rc = copy_out(h, accepted, h->hist_a, (size_t)h->batch * h->hist_cap); if (rc) return rc; }
@@ -509,6 +608,7 @@ int pimpc_get_cache(pimpc_t h, void *M, void *H)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     if (h->cache_dirty) return fail(h, PIMPC_ESTATE, "cache not computed yet (call pimpc_solve first)");
     const size_t nst = (size_t)h->batch * h->N;
     if (M) { rc = copy_out(h, M, h->M, nst * h->nu * h->nu * h->esz); if (rc) return rc; }
@@ -520,6 +620,7 @@ int pimpc_reset(pimpc_t h)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     const int n = launch_zero_state(h);
     if (n < 0) return PIMPC_ECUDA;
     h->info.total_launches += n;
@@ -530,6 +631,7 @@ int pimpc_shift(pimpc_t h, int steps)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     if (steps < 0 || steps >= h->N) return fail(h, PIMPC_EINVAL, "shift: steps must be in [0, N)");
     if (steps == 0) return PIMPC_OK;
     const int n = launch_shift(h, steps);
@@ -542,12 +644,14 @@ int pimpc_sync(pimpc_t h)
 {
     int rc = check_handle(h);
     if (rc) return rc;
+    DeviceGuard guard(h);
     return deferred_error(h);
 }
 
 int pimpc_get_info(pimpc_t h, pimpc_info *info)
 {
     if (!h || !info) return fail(h, PIMPC_EINVAL, "null argument");
+    DeviceGuard guard(h);
     if (h->ev_pending && !h->poisoned) {
         PIMPC_CUDA_TRY(h, cudaEventSynchronize(h->ev[2]));
         float a = 0.f, b = 0.f;

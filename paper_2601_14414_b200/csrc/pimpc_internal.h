@@ -3,8 +3,11 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "../../include/pimpc.h"
+
+constexpr int PIMPC_MAX_NB = 160;        // nx + nu ceiling (the generic cache kernel keeps an nb x nb double matrix in shared memory)
 
 // Per-instance control block of Algorithm 1 (device memory, one per instance).
 // alpha, c_prev: state of the accept/restart test; kappa = (alpha_i-1)/alpha_{i+1}
@@ -65,6 +68,9 @@ struct pimpc_s {
     double rho = 1.0, eta = 0.999, c0 = 1.0;
     int hist_cap = 0;
     cudaStream_t stream = nullptr;
+    pimpc_tune tune{};                       // launch-shape overrides (opts.tune), all 0 = automatic
+    unsigned char *ws = nullptr;             // caller-provided workspace (opts.workspace) or null
+    size_t ws_bytes = 0, ws_used = 0;
     int device = 0, sm_count = 0;
     size_t smem_optin = 0;
 
@@ -78,7 +84,7 @@ struct pimpc_s {
     void *H = nullptr, *M = nullptr, *S = nullptr, *X = nullptr, *DU = nullptr;
     InstCtl *ctl = nullptr;
     double *partial = nullptr;
-    int nparts_cap = 0;
+    size_t partial_cap = 0;                  // bytes
     double *hist_c = nullptr;
     unsigned char *hist_a = nullptr;
     int *err = nullptr;
@@ -90,8 +96,8 @@ struct pimpc_s {
     // engine-private storage (packed blobs of the STREAM engine etc.)
     void *blob = nullptr;
     size_t blob_bytes = 0;
-    double *spartial = nullptr;              // [2][grid][MAXI] partial sums of c of the STREAM engine
-    size_t spartial_cap = 0;
+    double *spartial = nullptr;              // [2][batch][span] partial sums of c of the STREAM engine
+    size_t spartial_cap = 0;                 // bytes
     bool blob_dirty = true;
     void *stage_buf = nullptr;               // device staging of results bound for host memory (grown on demand, kept)
     size_t stage_bytes = 0;
@@ -101,7 +107,12 @@ struct pimpc_s {
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // before cache kernel, before iteration, after iteration
     bool ev_pending = false, ev_setup = false;
 
-    bool cache_dirty = true;
+    bool cache_dirty = true;                 // every stage of the cache {M_k, H_k} must be recomputed
+    std::vector<int> dirty_stages;           // else: flattened (b * N + k) cache entries touched by pimpc_set_stage
+    double *res_part = nullptr;              // partial sums of r_prim2 (k_rprim), [batch][chunks]
+    size_t res_part_cap = 0;
+    int *dirty_dev = nullptr;                // device copy of dirty_stages
+    size_t dirty_cap = 0;
     size_t device_bytes = 0;
     pimpc_info info{};
     std::string errmsg;
@@ -111,7 +122,7 @@ struct pimpc_s {
 // ---- kernels / engine entry points (each returns the number of kernels it launched, <0 on error) ----
 template <typename T> Prob<T> make_prob(pimpc_s *h, double tol);
 
-int launch_setup(pimpc_s *h);                       // a0: cache {M_k, H_k}
+int launch_setup(pimpc_s *h, const int *list_dev, int nlist);   // a0: cache {M_k, H_k} of every stage (list_dev = null) or of the listed ones
 int launch_begin(pimpc_s *h);                       // Alg. 1 input: alpha=1, c_prev=c0, hats=iterates
 int run_staged(pimpc_s *h, int iters, double tol);  // v0 engine
 int run_resident(pimpc_s *h, int iters, double tol);
@@ -125,6 +136,10 @@ int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res_dev)
 int launch_state_io(pimpc_s *h, int which, void *buf_dev, int set);
 int launch_zero_state(pimpc_s *h);
 int launch_shift(pimpc_s *h, int steps);              // warm-start shift of the current iterate (reading R18)
+
+// (Re)allocate an engine-private device buffer of at least `bytes` (kept if large enough); accounts device_bytes; a failed
+// cudaMalloc returns PIMPC_ENOMEM without poisoning the handle.
+int pimpc_grow(pimpc_s *h, void **ptr, size_t *cap, size_t bytes);
 
 #define PIMPC_CUDA_TRY(h, expr)                                                         \
     do {                                                                                \

@@ -28,15 +28,23 @@ X, Z, V, TH, BE, LA, D, DE, DU = range(9)
 STATE = {"X": X, "Z": Z, "V": V, "TH": TH, "BE": BE, "LA": LA, "D": D, "DE": DE, "DU": DU}
 
 
+class pimpc_tune(ctypes.Structure):
+    _fields_ = [("grid", ctypes.c_int), ("ctas_per_sm", ctypes.c_int), ("ring_slots", ctypes.c_int),
+                ("stages_per_group", ctypes.c_int), ("cluster", ctypes.c_int), ("rows_per_lane", ctypes.c_int),
+                ("lookahead", ctypes.c_int), ("reserved_", ctypes.c_int)]
+
+
 class pimpc_opts(ctypes.Structure):
     _fields_ = [("dtype", ctypes.c_int), ("engine", ctypes.c_int), ("rho", ctypes.c_double),
                 ("eta", ctypes.c_double), ("c0", ctypes.c_double), ("history", ctypes.c_int),
-                ("stream", ctypes.c_void_p)]
+                ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
+                ("tune", pimpc_tune)]
 
 
 class pimpc_result(ctypes.Structure):
-    _fields_ = [("c", ctypes.c_double), ("alpha", ctypes.c_double), ("iters", ctypes.c_int),
-                ("restarts", ctypes.c_int), ("converged", ctypes.c_int), ("pad_", ctypes.c_int)]
+    _fields_ = [("c", ctypes.c_double), ("alpha", ctypes.c_double), ("r_prim2", ctypes.c_double),
+                ("r_dual2", ctypes.c_double), ("iters", ctypes.c_int), ("restarts", ctypes.c_int),
+                ("converged", ctypes.c_int), ("pad_", ctypes.c_int)]
 
 
 class pimpc_info(ctypes.Structure):
@@ -46,13 +54,19 @@ class pimpc_info(ctypes.Structure):
                 ("iter_ms", ctypes.c_double)]
 
 
-RESULT_DTYPE = np.dtype([("c", "f8"), ("alpha", "f8"), ("iters", "i4"), ("restarts", "i4"),
-                         ("converged", "i4"), ("pad_", "i4")])
+class pimpc_peaks(ctypes.Structure):
+    _fields_ = [("ffma_tflops", ctypes.c_double), ("ffma2_tflops", ctypes.c_double), ("dfma_tflops", ctypes.c_double),
+                ("smem_gbs", ctypes.c_double), ("sm_count", ctypes.c_int), ("pad_", ctypes.c_int)]
+
+
+RESULT_DTYPE = np.dtype([("c", "f8"), ("alpha", "f8"), ("r_prim2", "f8"), ("r_dual2", "f8"), ("iters", "i4"),
+                         ("restarts", "i4"), ("converged", "i4"), ("pad_", "i4")])
 
 # name -> (restype, argtypes); every symbol include/pimpc.h declares
 _vp, _i, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
 SYMBOLS = {
     "pimpc_version": (ctypes.c_char_p, []),
+    "pimpc_measure_peaks": (_i, [ctypes.POINTER(pimpc_peaks), _vp]),
     "pimpc_default_opts": (None, [ctypes.POINTER(pimpc_opts)]),
     "pimpc_workspace_bytes": (ctypes.c_size_t, [_i, _i, _i, _i, ctypes.POINTER(pimpc_opts)]),
     "pimpc_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i, ctypes.POINTER(pimpc_opts)]),
@@ -121,7 +135,9 @@ class Solver:
     """One libpimpc handle.  Methods mirror the C entry points (without the `pimpc_` prefix)."""
 
     def __init__(self, nx, nu, N, batch=1, *, dtype="f64", engine="auto", rho=1.0, eta=0.999, c0=1.0,
-                 history=0, stream=None):
+                 history=0, stream=None, workspace=None, tune=None):
+        """workspace: a CUDA tensor (uint8 / any dtype) of at least workspace_bytes(...) bytes, kept alive by the
+        Solver; tune: dict of pimpc_tune fields (launch-shape overrides, see include/pimpc.h)."""
         self.lib = load()
         self.nx, self.nu, self.N, self.batch, self.nb = nx, nu, N, batch, nx + nu
         self.dtype = dtype
@@ -135,7 +151,14 @@ class Solver:
         if stream is None and torch is not None and torch.cuda.is_available():
             stream = torch.cuda.current_stream().cuda_stream
         o.stream = stream
-        self._keep = []          # host arrays that must outlive an asynchronous call
+        self._workspace = workspace              # keeps the caller's tensor alive as long as the handle
+        if workspace is not None:
+            o.workspace = workspace.data_ptr()
+            o.workspace_bytes = workspace.numel() * workspace.element_size()
+        for k, v in (tune or {}).items():
+            if not hasattr(o.tune, k):
+                raise KeyError(f"unknown pimpc_tune field {k!r}")
+            setattr(o.tune, k, int(v))
         h = ctypes.c_void_p()
         rc = self.lib.pimpc_create(ctypes.byref(h), nx, nu, N, batch, ctypes.byref(o))
         if rc != OK:
@@ -248,6 +271,23 @@ class Solver:
         info = pimpc_info()
         self._ck(self.lib.pimpc_get_info(self.h, ctypes.byref(info)))
         return {f: getattr(info, f) for f, _ in pimpc_info._fields_}
+
+
+def workspace_bytes(nx, nu, N, batch=1, *, dtype="f64", history=0) -> int:
+    o = pimpc_opts()
+    load().pimpc_default_opts(ctypes.byref(o))
+    o.dtype = F64 if dtype == "f64" else F32
+    o.history = int(history)
+    return int(load().pimpc_workspace_bytes(nx, nu, N, batch, ctypes.byref(o)))
+
+
+def measure_peaks(stream=None) -> dict:
+    """pimpc_measure_peaks on the current device: measured FP32 / FP64 FMA TFLOP/s and shared-memory GB/s."""
+    pk = pimpc_peaks()
+    rc = load().pimpc_measure_peaks(ctypes.byref(pk), stream)
+    if rc != OK:
+        raise PimpcError(rc, "pimpc_measure_peaks failed")
+    return {f: getattr(pk, f) for f, _ in pimpc_peaks._fields_ if f != "pad_"}
 
 
 def version() -> str:

@@ -35,10 +35,23 @@ def test_every_declared_symbol_is_exported_and_bound(lib):
 
 def test_struct_layouts_match_header(lib):
     from paper_2601_14414_b200 import pimpc
-    assert ctypes.sizeof(pimpc.pimpc_result) == 32 and pimpc.RESULT_DTYPE.itemsize == 32
+    assert ctypes.sizeof(pimpc.pimpc_result) == 48 and pimpc.RESULT_DTYPE.itemsize == 48
+    for f, _ in pimpc.pimpc_result._fields_:
+        assert getattr(pimpc.pimpc_result, f).offset == pimpc.RESULT_DTYPE.fields[f][1]
+    assert ctypes.sizeof(pimpc.pimpc_tune) == 32
     o = pimpc.pimpc_opts()
+    ctypes.memset(ctypes.byref(o), 0xFF, ctypes.sizeof(o))
     lib.pimpc_default_opts(ctypes.byref(o))
     assert (o.dtype, o.engine, o.rho, o.eta, o.c0, o.history) == (0, 0, 1.0, 0.999, 1.0, 0)
+    assert o.workspace is None and o.workspace_bytes == 0
+    assert all(getattr(o.tune, f) == 0 for f, _ in pimpc.pimpc_tune._fields_)
+    # the header's struct members, in order, are the binding's fields
+    src = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "pimpc.h")).read(), flags=re.S)
+    for cname, cls in (("pimpc_tune", pimpc.pimpc_tune), ("pimpc_opts", pimpc.pimpc_opts), ("pimpc_result", pimpc.pimpc_result),
+                       ("pimpc_info", pimpc.pimpc_info), ("pimpc_peaks", pimpc.pimpc_peaks)):
+        body = re.search(r"typedef struct \{([^{}]*)\} " + cname + ";", src).group(1)
+        names = [re.search(r"(\w+)\s*$", part).group(1) for decl in body.split(";") if decl.strip() for part in decl.split(",")]
+        assert names == [f for f, _ in cls._fields_], (cname, names)
     assert b"sm_100a" in lib.pimpc_version()
 
 
@@ -46,7 +59,9 @@ def test_workspace_bytes_and_argument_validation(lib):
     from paper_2601_14414_b200 import pimpc
     o = pimpc.pimpc_opts(); lib.pimpc_default_opts(ctypes.byref(o))
     assert lib.pimpc_workspace_bytes(0, 1, 1, 1, ctypes.byref(o)) == 0
-    assert lib.pimpc_workspace_bytes(100, 60, 1, 1, ctypes.byref(o)) == 0
+    assert lib.pimpc_workspace_bytes(100, 61, 1, 1, ctypes.byref(o)) == 0        # nx + nu > 160
+    assert lib.pimpc_workspace_bytes(100, 30, 1, 1, ctypes.byref(o)) > 0         # the paper's largest Table-I shape
+    assert lib.pimpc_workspace_bytes(2, 1, 3, 70000, ctypes.byref(o)) == 0       # batch > 65535
     w64 = lib.pimpc_workspace_bytes(12, 4, 50, 4096, ctypes.byref(o))
     o.dtype = pimpc.F32
     w32 = lib.pimpc_workspace_bytes(12, 4, 50, 4096, ctypes.byref(o))

@@ -257,6 +257,31 @@ def test_convergence_residuals_and_stationarity(oracle):
         xb = r.X[k]
 
 
+def test_residual_halves_match_the_definition_of_the_primal_residual(oracle):
+    """PAPER.md:259-263, (14a), (15c): the primal half of c is rho ||F p + G q - h||^2.  The oracle forms it from the
+    dual differences s^{i+1} - shat^i; here it is rebuilt from the DEFINITION of the consensus constraints of
+    Problem (11) on the returned X, DU, Z, V[, D] with dense Abar, Bbar -- a different formula that
+    agrees only if every dual update (step 3) is the running sum of its constraint residual."""
+    for du_bound, iters in ((None, 37), (0.3, 52)):
+        p = wl.random_ltv(3, 2, 6, 1, seed=21, affine=True, u_prev=True, qbar=True, bounds=0.7, du_bound=du_bound)
+        r = _solve(oracle, p, max_iters=iters, tol=0.0)
+        nx, nu, N = p.nx, p.nu, p.N
+        tot = 0.0
+        xk = np.concatenate([p.x0[0], p.u_prev[0]])
+        for k in range(N):
+            Ab = np.block([[p.A[0, k], p.B[0, k]], [np.zeros((nu, nx)), np.eye(nu)]])
+            Bb = np.vstack([p.B[0, k], np.eye(nu)])
+            eb = np.concatenate([p.e[0, k], np.zeros(nu)])
+            tot += np.sum((r.X[k] - r.Z[k]) ** 2) + np.sum((Bb @ r.DU[k] - r.V[k]) ** 2)
+            tot += np.sum((r.Z[k] - Ab @ xk - r.V[k] - eb) ** 2)
+            if du_bound is not None:
+                tot += np.sum((r.DU[k] - r.D[k]) ** 2)
+            xk = r.X[k]
+        assert abs(p.rho * tot - r.r_prim2) <= 1e-12 * max(1.0, r.r_prim2)
+        assert abs(r.r_prim2 + r.r_dual2 - r.c_last) <= 1e-13 * max(1.0, r.c_last)
+        assert r.r_prim2 > 0 and r.r_dual2 > 0
+
+
 def test_warm_start_is_a_fresh_alg1_invocation(oracle):
     """the output iterates seed the next invocation with hats = iterates, alpha_0 = 1."""
     p = wl.quadrotor_ltv(6, 1)
