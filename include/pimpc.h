@@ -156,7 +156,7 @@ int pimpc_set_stages(pimpc_t h, const void *A, const void *B, const void *e);
 /* Cost.  Q [nx][nx] = C'W_y C and R [nu][nu] = W_u symmetric PSD.
  * P [nx][nx] or NULL: terminal weight used instead of Q at stage N-1 (R14; NULL = Q).
  * Wdu [nu][nu] or NULL: weight on Delta u (R13; NULL = 0).
- * qbar [nx+nu] or NULL: linear term col(C'W_y r_y, W_u r_u) (NULL = 0).
+ * qbar [nx+nu] or NULL: linear term col(C'W_y r_y, W_u r_u) (NULL = 0); replaces per-stage linear terms.
  * per_instance != 0: each array has a leading [batch] dimension. */
 int pimpc_set_cost(pimpc_t h, const void *Q, const void *R, const void *P, const void *Wdu,
                    const void *qbar, int per_instance);
@@ -167,6 +167,35 @@ int pimpc_set_cost(pimpc_t h, const void *Q, const void *R, const void *P, const
  * per_instance != 0: leading [batch] dimension.  EINVAL if any lo > hi or a NaN. */
 int pimpc_set_bounds(pimpc_t h, const void *lo, const void *hi, const void *du_lo, const void *du_hi,
                      int per_instance);
+
+/* Tracking cost of problem (1a): 1/2 ||C x_{k+1} - r_y||^2_{W_y} + 1/2 ||u_k - r_u||^2_{W_u}.  Forms, on the
+ * device and in double precision,  Q = C'W_y C,  R = W_u,  qbar = col(C'W_y r_y, W_u r_u) and installs them
+ * as the (shared) cost of the handle, like pimpc_set_cost(Q, R, P = NULL, Wdu = unchanged, qbar).
+ * C [ny][nx], Wy [ny][ny], Wu [nu][nu] symmetric PSD; ry, ru may be NULL (= 0).
+ * per_stage == 0: ry [ny], ru [nu].  per_stage != 0: time-varying references ry [N][ny] (for x_1..x_N), ru [N][nu] (for
+ * u_0..u_{N-1}); qbar then differs per stage (only the STAGED and STREAM engines take per-stage terms).
+ * EINVAL: ny <= 0, ny > 160, C / Wy / Wu NULL, per-instance cost already set. */
+int pimpc_set_tracking(pimpc_t h, int ny, const void *C, const void *Wy, const void *Wu, const void *ry, const void *ru,
+                       int per_stage);
+
+/* Per-stage boxes and linear terms (stage-dependent sets X_k, U_k and references; problem (1) with stage-dependent data):
+ * lo, hi [N][nb] (row k bounds (x_{k+1}; u_k)) replace the shared box of pimpc_set_bounds; qbar [N][nb] replaces the
+ * shared linear term.  lo and hi come together; any argument NULL = that item is not per-stage (back to the shared one).
+ * per_instance != 0: leading [batch] dimension.  Only the STAGED and STREAM engines take per-stage terms (AUTO picks
+ * among them).  EINVAL if any lo > hi or a NaN. */
+int pimpc_set_stage_terms(pimpc_t h, const void *lo, const void *hi, const void *qbar, int per_instance);
+
+/* General closed convex set for part of z_{k+1} (Theorem 1: the z-update is Proj of the same argument
+ * for ANY closed convex set).  The components [i0, i0 + len) of every (x_{k+1}; u_k) are projected onto
+ *   PIMPC_SET_HALFSPACE  {s : a's <= b}        PIMPC_SET_HYPERPLANE {s : a's = b}
+ *   PIMPC_SET_SOC        {(s, r) : ||s||_2 <= r}, r = the last of the len components
+ *   PIMPC_SET_L1BALL     {s : ||s||_1 <= b}
+ * (closed forms of [22, Ch. 6]) instead of being clipped; the other components keep their box: the
+ * constraint set is the product box x set.  a [len] (halfspace, hyperplane; element type of the handle; else NULL),
+ * b = offset or radius.  PIMPC_SET_NONE removes the set.  Shared by all stages and instances.  Only the STAGED and STREAM
+ * engines take a general set.  EINVAL: bad kind or range, a missing or all zero, b < 0 for the l1 ball, len < 2 for the cone. */
+enum { PIMPC_SET_NONE = 0, PIMPC_SET_HALFSPACE = 1, PIMPC_SET_HYPERPLANE = 2, PIMPC_SET_SOC = 3, PIMPC_SET_L1BALL = 4 };
+int pimpc_set_constraint(pimpc_t h, int kind, int i0, int len, const void *a, double b);
 
 /* x0 [batch][nx] = x(t); u_prev [batch][nu] = u(t-1) or NULL (= 0)  (xbar_0, R10). */
 int pimpc_set_x0(pimpc_t h, const void *x0, const void *u_prev);

@@ -18,6 +18,11 @@
  * fusion or reordering.  Where the paper is garbled or silent the reading of
  * DESIGN.md "Readings of the paper" (R1..R17) is taken; each is marked below.
  *
+ * Extensions: the other projections the paper lists (halfspace, hyperplane, second-order cone,
+ * l1 ball), per-stage boxes and linear terms, and the tracking cost (1a) -> (Q, R, qbar).
+ * Their pins: variational inequality + brute-force nearest point per set, scipy SLSQP on the QP with the set, and
+ * a least-squares KKT solve of the tracking problem.
+ *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): dense KKT solve of QP (1)
  * (unconstrained LTV, affine e_k, u_prev), brute-force active-set enumeration
  * (u-, x- and du-bounds active), the closed form c^1, the SURVEY P-tiny
@@ -101,6 +106,149 @@ static double clip(double t, double lo, double hi)
 
 static double sq(double x) { return x * x; }
 
+/* ---- projections onto the closed convex sets the paper lists for Proj (closed forms of [22, Ch. 6]) ----
+ * Each maps t (n entries) to the nearest point of the set, written to out (out may alias t). */
+
+/* halfspace {x : a^T x <= b}: t if it is inside, else t - ((a^T t - b) / ||a||^2) a */
+static void proj_halfspace(int n, const double *t, const double *a, double b, double *out)
+{
+    double at = 0.0, aa = 0.0;
+    for (int i = 0; i < n; ++i) { at += a[i] * t[i]; aa += a[i] * a[i]; }
+    double s = (at > b && aa > 0.0) ? (at - b) / aa : 0.0;
+    for (int i = 0; i < n; ++i) out[i] = t[i] - s * a[i];
+}
+
+/* affine hyperplane {x : a^T x = b}: t - ((a^T t - b) / ||a||^2) a */
+static void proj_hyperplane(int n, const double *t, const double *a, double b, double *out)
+{
+    double at = 0.0, aa = 0.0;
+    for (int i = 0; i < n; ++i) { at += a[i] * t[i]; aa += a[i] * a[i]; }
+    double s = aa > 0.0 ? (at - b) / aa : 0.0;
+    for (int i = 0; i < n; ++i) out[i] = t[i] - s * a[i];
+}
+
+/* second-order cone {(x, r) : ||x||_2 <= r}, t = (x (n-1 entries), r):
+ * inside: t;  ||x|| <= -r (polar cone): 0;  else ((||x|| + r) / 2) (x / ||x||, 1) */
+static void proj_soc(int n, const double *t, double *out)
+{
+    double nx2 = 0.0, r = t[n - 1];
+    for (int i = 0; i < n - 1; ++i) nx2 += t[i] * t[i];
+    double nx = sqrt(nx2);
+    if (nx <= r) { for (int i = 0; i < n; ++i) out[i] = t[i]; return; }
+    if (nx <= -r) { for (int i = 0; i < n; ++i) out[i] = 0.0; return; }
+    double s = 0.5 * (nx + r);
+    for (int i = 0; i < n - 1; ++i) out[i] = s * t[i] / nx;
+    out[n - 1] = s;
+}
+
+/* l1 ball {x : ||x||_1 <= r}, r >= 0: t if inside, else the soft threshold sign(t_i) max(|t_i| - tau, 0) with the tau
+ * that makes the l1 norm r: sort |t| in descending order u_1 >= u_2 >= ..., m = the largest j with
+ * u_j > (u_1 + ... + u_j - r) / j, tau = (u_1 + ... + u_m - r) / m. */
+static void proj_l1ball(int n, const double *t, double r, double *out)
+{
+    double l1 = 0.0;
+    for (int i = 0; i < n; ++i) l1 += fabs(t[i]);
+    if (l1 <= r) { for (int i = 0; i < n; ++i) out[i] = t[i]; return; }
+    double *u = (double *)malloc((size_t)n * sizeof(double));
+    for (int i = 0; i < n; ++i) u[i] = fabs(t[i]);
+    for (int i = 1; i < n; ++i) {                     /* insertion sort, descending */
+        double v = u[i]; int j = i - 1;
+        while (j >= 0 && u[j] < v) { u[j + 1] = u[j]; --j; }
+        u[j + 1] = v;
+    }
+    double cs = 0.0, tau = 0.0;
+    for (int j = 1; j <= n; ++j) {
+        cs += u[j - 1];
+        double cand = (cs - r) / j;
+        if (u[j - 1] > cand) tau = cand;
+    }
+    free(u);
+    for (int i = 0; i < n; ++i) {
+        double m = fabs(t[i]) - tau;
+        out[i] = m > 0.0 ? (t[i] > 0.0 ? m : -m) : 0.0;
+    }
+}
+
+/* Optional extensions of problem (1).  All pointers may be NULL. */
+enum { PIMPC_ORACLE_SET_NONE = 0, PIMPC_ORACLE_SET_HALFSPACE = 1, PIMPC_ORACLE_SET_HYPERPLANE = 2,
+       PIMPC_ORACLE_SET_SOC = 3, PIMPC_ORACLE_SET_L1BALL = 4 };
+typedef struct {
+    int set_kind;            /* which closed convex set the components [set_i0, set_i0 + set_len) of z_{k+1} lie in;
+                                the other components stay in the box [lo, hi]: Xbar = box x set (a product, so the
+                                projection is the product of the projections)                                        */
+    int set_i0, set_len;
+    const double *set_a;     /* [set_len] normal vector a of the halfspace / hyperplane                              */
+    double set_b;            /* offset b (halfspace, hyperplane) or radius r (l1 ball)                               */
+    const double *lo_k, *hi_k;   /* per-stage boxes [N][nb] replacing lo / hi (x_{k+1} in X_k, u_k in U_k)           */
+    const double *qbar_k;        /* per-stage linear terms [N][nb] replacing qbar (time-varying references r_y, r_u) */
+} pimpc_oracle_ext;
+
+/* Proj onto Xbar of one stage: t -> z (nb entries) */
+static void proj_xbar(int nb, const double *t, const double *lo, const double *hi, const pimpc_oracle_ext *x, double *z)
+{
+    for (int i = 0; i < nb; ++i) z[i] = clip(t[i], lo[i], hi[i]);
+    if (!x || x->set_kind == PIMPC_ORACLE_SET_NONE) return;
+    const int i0 = x->set_i0, n = x->set_len;
+    switch (x->set_kind) {
+    case PIMPC_ORACLE_SET_HALFSPACE: proj_halfspace(n, t + i0, x->set_a, x->set_b, z + i0); break;
+    case PIMPC_ORACLE_SET_HYPERPLANE: proj_hyperplane(n, t + i0, x->set_a, x->set_b, z + i0); break;
+    case PIMPC_ORACLE_SET_SOC: proj_soc(n, t + i0, z + i0); break;
+    case PIMPC_ORACLE_SET_L1BALL: proj_l1ball(n, t + i0, x->set_b, z + i0); break;
+    default: break;
+    }
+}
+
+/* The projections alone, for the pins of tests/test_oracle_pins.py: kind as above, a may be NULL. */
+int pimpc_oracle_project(int kind, int n, const double *t, const double *a, double b, double *out)
+{
+    if (n <= 0 || !t || !out) return -1;
+    switch (kind) {
+    case PIMPC_ORACLE_SET_HALFSPACE: if (!a) return -1; proj_halfspace(n, t, a, b, out); return 0;
+    case PIMPC_ORACLE_SET_HYPERPLANE: if (!a) return -1; proj_hyperplane(n, t, a, b, out); return 0;
+    case PIMPC_ORACLE_SET_SOC: proj_soc(n, t, out); return 0;
+    case PIMPC_ORACLE_SET_L1BALL: if (b < 0.0) return -1; proj_l1ball(n, t, b, out); return 0;
+    default: return -1;
+    }
+}
+
+/* Tracking cost of problem (1a) in the form of problem (11):
+ *   Q = C^T W_y C [nx][nx],  R = W_u [nu][nu],  qbar = col(C^T W_y r_y, W_u r_u) [nx+nu];  C [ny][nx], W_y [ny][ny]. */
+int pimpc_oracle_tracking(int nx, int nu, int ny, const double *C, const double *Wy, const double *Wu,
+                          const double *ry, const double *ru, double *Q, double *R, double *qbar)
+{
+    if (nx <= 0 || nu <= 0 || ny <= 0 || !C || !Wy || !Wu) return -1;
+    double *WC = (double *)calloc((size_t)ny * nx, sizeof(double));      /* W_y C */
+    double *Wr = (double *)calloc((size_t)ny, sizeof(double));           /* W_y r_y */
+    if (!WC || !Wr) { free(WC); free(Wr); return -2; }
+    for (int i = 0; i < ny; ++i) {
+        for (int j = 0; j < nx; ++j) {
+            double s = 0.0;
+            for (int p = 0; p < ny; ++p) s += Wy[i * ny + p] * C[p * nx + j];
+            WC[i * nx + j] = s;
+        }
+        double s = 0.0;
+        for (int p = 0; p < ny; ++p) s += Wy[i * ny + p] * (ry ? ry[p] : 0.0);
+        Wr[i] = s;
+    }
+    for (int i = 0; i < nx; ++i) {
+        for (int j = 0; j < nx; ++j) {
+            double s = 0.0;
+            for (int p = 0; p < ny; ++p) s += C[p * nx + i] * WC[p * nx + j];
+            Q[i * nx + j] = s;
+        }
+        double s = 0.0;
+        for (int p = 0; p < ny; ++p) s += C[p * nx + i] * Wr[p];
+        qbar[i] = s;
+    }
+    for (int i = 0; i < nu; ++i) {
+        double s = 0.0;
+        for (int j = 0; j < nu; ++j) { R[i * nu + j] = Wu[i * nu + j]; s += Wu[i * nu + j] * (ru ? ru[j] : 0.0); }
+        qbar[nx + i] = s;
+    }
+    free(WC); free(Wr);
+    return 0;
+}
+
 /*
  * One invocation of Algorithm 1 for ONE problem instance.
  *
@@ -130,6 +278,7 @@ static double sq(double x) { return x * x; }
  *   r_parts [2] or NULL: the two halves of c_last:
  *       r_parts[0] = rho ||s^{i+1} - shat^i||^2  (primal residual F p + G q - h, by (15c))
  *       r_parts[1] = rho ||G (q^{i+1} - qhat^i)||^2  (dual residual)
+ *   ext or NULL: general convex set on part of z, per-stage boxes, per-stage linear terms (see pimpc_oracle_ext)
  * Returns 0, -1 bad argument, -2 out of memory, -5 matrix not positive definite.
  */
 int pimpc_oracle_solve(
@@ -145,7 +294,7 @@ int pimpc_oracle_solve(
     double *Z, double *V, double *TH, double *BE, double *LA, double *D, double *DE,
     double *X, double *DU,
     double *c_hist, unsigned char *acc_hist,
-    int *info, double *c_last, double *r_parts)
+    int *info, double *c_last, double *r_parts, const pimpc_oracle_ext *ext)
 {
     if (nx <= 0 || nu <= 0 || N <= 0 || !(rho > 0.0) || max_iters < 0) return -1;
     if ((du_lo == NULL) != (du_hi == NULL)) return -1;
@@ -177,6 +326,12 @@ int pimpc_oracle_solve(
     double *Dn = (double *)calloc(szu, sizeof(double)), *DEn = (double *)calloc(szu, sizeof(double));
     double *t1 = (double *)calloc((size_t)nb, sizeof(double)), *t2 = (double *)calloc((size_t)nb, sizeof(double));
     double *t3 = (double *)calloc((size_t)nb, sizeof(double)), *t4 = (double *)calloc((size_t)nb, sizeof(double));
+    double *va = (double *)calloc((size_t)nb, sizeof(double)), *vb = (double *)calloc((size_t)nb, sizeof(double));
+    double *vt = (double *)calloc((size_t)nb, sizeof(double)), *vz = (double *)calloc((size_t)nb, sizeof(double));
+    if (ext && ext->set_kind != PIMPC_ORACLE_SET_NONE &&
+        (ext->set_i0 < 0 || ext->set_len <= 0 || ext->set_i0 + ext->set_len > nb ||
+         ((ext->set_kind == PIMPC_ORACLE_SET_HALFSPACE || ext->set_kind == PIMPC_ORACLE_SET_HYPERPLANE) && !ext->set_a))) { rc = -1; goto done; }
+    if (!va || !vb || !vt || !vz) { rc = -2; goto done; }
     if (!Abar || !Bbar || !ebar || !Qbar || !QbarN || !qb || !xbar0 || !M || !H || !S || !Zh || !Vh ||
         !THh || !BEh || !LAh || !Dh || !DEh || !Zn || !Vn || !THn || !BEn || !LAn || !Dn || !DEn ||
         !t1 || !t2 || !t3 || !t4) { rc = -2; goto done; }
@@ -257,7 +412,8 @@ int pimpc_oracle_solve(
             /* h_k = qbar + rho (zhat_{k+1} - thetahat_k)
                      [+ rho Abar_{k+1}^T (zhat_{k+2} - vhat_{k+1} - ebar_{k+1} + lambdahat_{k+1})]   (R2) */
             for (int i = 0; i < nb; ++i)
-                t3[i] = qb[i] + rho * (Zh[(size_t)k * nb + i] - THh[(size_t)k * nb + i]);
+                t3[i] = ((ext && ext->qbar_k) ? ext->qbar_k[(size_t)k * nb + i] : qb[i])
+                      + rho * (Zh[(size_t)k * nb + i] - THh[(size_t)k * nb + i]);
             if (k < N - 1) {
                 const double *Ab1 = Abar + (size_t)(k + 1) * nb * nb;
                 for (int i = 0; i < nb; ++i)
@@ -277,10 +433,17 @@ int pimpc_oracle_solve(
             matvec(nb, nb, Ab, xk, t2);                        /* Abar_k xbar_k   */
             for (int i = 0; i < nb; ++i) {
                 size_t q = (size_t)k * nb + i;
-                double a = t1[i] + BEh[q];                     /* Bbar du + betahat            */
-                double b = t2[i] + ebar[q] - LAh[q];           /* Abar xbar + ebar - lambdahat */
-                double gamma = a - b;
-                double zn = clip((2.0 * (X[q] + THh[q] + b) + gamma) / 3.0, lo[i], hi[i]);
+                va[i] = t1[i] + BEh[q];                        /* a = Bbar du + betahat            */
+                vb[i] = t2[i] + ebar[q] - LAh[q];              /* b = Abar xbar + ebar - lambdahat */
+                double gamma = va[i] - vb[i];
+                vt[i] = (2.0 * (X[q] + THh[q] + vb[i]) + gamma) / 3.0;      /* argument of Proj */
+            }
+            /* z_{k+1} = Proj_Xbar(.) (Thm 1: exact for any closed convex set) */
+            proj_xbar(nb, vt, (ext && ext->lo_k) ? ext->lo_k + (size_t)k * nb : lo,
+                      (ext && ext->hi_k) ? ext->hi_k + (size_t)k * nb : hi, ext, vz);
+            for (int i = 0; i < nb; ++i) {
+                size_t q = (size_t)k * nb + i;
+                double a = va[i], b = vb[i], gamma = a - b, zn = vz[i];
                 double vn = 0.5 * (zn + gamma);
                 Zn[q] = zn; Vn[q] = vn;
                 THn[q] = THh[q] + X[q] - zn;
@@ -356,7 +519,7 @@ done:
     free(M); free(H); free(S);
     free(Zh); free(Vh); free(THh); free(BEh); free(LAh); free(Dh); free(DEh);
     free(Zn); free(Vn); free(THn); free(BEn); free(LAn); free(Dn); free(DEn);
-    free(t1); free(t2); free(t3); free(t4);
+    free(t1); free(t2); free(t3); free(t4); free(va); free(vb); free(vt); free(vz);
     return rc;
 }
 

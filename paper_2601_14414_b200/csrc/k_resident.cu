@@ -424,25 +424,19 @@ int launch_resident(pimpc_s *h, int iters, double tol, int nwarps)
     return 1;
 }
 
-// instantiation table: (dtype, nx, nu) -> rows per lane, stages per warp, thread ceilings
-struct ResidentPlan { int spw; int max_stages; };
-
-bool plan_for(const pimpc_s *h, ResidentPlan *pl)
-{
-    if (h->dtype == PIMPC_F32 && h->nx == 12 && h->nu == 4) { *pl = {2, 64}; return true; }
-    if (h->dtype == PIMPC_F64 && h->nx == 4 && h->nu == 2) { *pl = {4, 64}; return true; }
-    if (h->dtype == PIMPC_F32 && h->nx == 4 && h->nu == 2) { *pl = {4, 128}; return true; }
-    return false;
-}
-
 } // namespace
+
+// The one-row-per-lane kernel above serves fp32 (12, 4) horizons beyond the 13 warps of the two-rows-per-lane kernel
+// (53 <= N <= 64) and opts.tune.rows_per_lane = 1; every other RESIDENT solve runs k_res2 (k_resident2.cu).
+static bool one_row_shape(const pimpc_s *h) { return h->dtype == PIMPC_F32 && h->nx == 12 && h->nu == 4 && h->N <= 64; }
 
 bool resident_supported(const pimpc_s *h, std::string *why)
 {
-    ResidentPlan pl;
-    if (!plan_for(h, &pl)) { if (why) *why = "no register-resident instantiation for this (dtype, nx, nu)"; return false; }
-    if (h->N > pl.max_stages) { if (why) *why = "horizon exceeds what one CTA keeps in registers"; return false; }
-    return true;
+    int nxp, nup, maxn;
+    if (resident2_plan(h, &nxp, &nup, &maxn) && h->N <= maxn) return true;
+    if (one_row_shape(h)) return true;
+    if (why) *why = "no register-resident instantiation for this (dtype, nx, nu, N)";
+    return false;
 }
 
 int ensure_alpha_table(pimpc_s *h, int iters)
@@ -464,24 +458,17 @@ int ensure_alpha_table(pimpc_s *h, int iters)
 
 int run_resident(pimpc_s *h, int iters, double tol)
 {
-    ResidentPlan pl;
-    if (!plan_for(h, &pl) || h->N > pl.max_stages) { h->errmsg = "RESIDENT engine not applicable"; return PIMPC_EINVAL; }
+    if (!resident_supported(h, nullptr)) { h->errmsg = "RESIDENT engine not applicable"; return PIMPC_EINVAL; }
     const int launches = ensure_alpha_table(h, iters);
     if (launches < 0) return launches;
-    int nwarps = (h->N + pl.spw - 1) / pl.spw;
-    int n;
-    if (h->dtype == PIMPC_F32 && h->nx == 12 && h->tune.rows_per_lane != 1 && h->N <= 56) {   // tune: 1 = one row per lane (16 lanes per stage)
-        // two rows per lane, 8 lanes per stage: half the broadcast loads per FMA.  C4 on B200: 8.23 ms, against 9.11 ms
-        // with one row per lane and 8.94 ms with four
-        nwarps = (h->N + 3) / 4;
-        n = launch_resident<float, 12, 4, 2, 448>(h, iters, tol, nwarps);
-    } else if (h->dtype == PIMPC_F32 && h->nx == 12) {
+    int nxp, nup, maxn, n;
+    const bool two = resident2_plan(h, &nxp, &nup, &maxn) && h->N <= maxn;
+    if (two && !(h->tune.rows_per_lane == 1 && one_row_shape(h))) {
+        n = run_resident2(h, iters, tol);
+    } else {
+        const int nwarps = (h->N + 1) / 2;                     // 16 lanes per stage, 2 stages per warp
         n = nwarps <= 25 ? launch_resident<float, 12, 4, 1, 800>(h, iters, tol, nwarps)
                          : launch_resident<float, 12, 4, 1, 1024>(h, iters, tol, nwarps);
-    } else if (h->dtype == PIMPC_F64) {
-        n = launch_resident<double, 4, 2, 1, 512>(h, iters, tol, nwarps);
-    } else {
-        n = launch_resident<float, 4, 2, 1, 1024>(h, iters, tol, nwarps);
     }
     return n < 0 ? n : n + launches;
 }

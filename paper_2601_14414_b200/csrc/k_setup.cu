@@ -247,6 +247,44 @@ __global__ void __launch_bounds__(128) k_setup_small(Prob<T> p, const int *__res
     else if (!ok) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
 }
 
+// Tracking cost (1a) -> the cost of problem (11): Q = C'W_y C, R = W_u, and for each of the nref
+// reference pairs qbar[k] = col(C'W_y r_y[k], W_u r_u[k]).  One thread per output element, double accumulation.
+template <typename T>
+__global__ void k_tracking(int nx, int nu, int ny, const T *__restrict__ C, const T *__restrict__ Wy, const T *__restrict__ Wu,
+                           const T *__restrict__ ry, const T *__restrict__ ru, int nref, T *__restrict__ Q, T *__restrict__ R,
+                           T *__restrict__ qbar)
+{
+    const int nb = nx + nu, nq = nx * nx, nr = nu * nu, total = nq + nr + nref * nb;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        if (idx < nq) {                                        // Q[i][j] = sum_{p,q} C[p][i] Wy[p][q] C[q][j]
+            const int i = idx / nx, j = idx - i * nx;
+            double s = 0.0;
+            for (int a = 0; a < ny; ++a) {
+                double w = 0.0;
+                for (int b = 0; b < ny; ++b) w += (double)Wy[a * ny + b] * (double)C[b * nx + j];
+                s += (double)C[a * nx + i] * w;
+            }
+            Q[idx] = (T)s;
+        } else if (idx < nq + nr) {
+            R[idx - nq] = Wu[idx - nq];
+        } else {
+            const int q = idx - nq - nr, k = q / nb, i = q - k * nb;
+            double s = 0.0;
+            if (i < nx) {                                      // (C'W_y r_y)_i
+                if (ry)
+                    for (int a = 0; a < ny; ++a) {
+                        double w = 0.0;
+                        for (int b = 0; b < ny; ++b) w += (double)Wy[a * ny + b] * (double)ry[k * ny + b];
+                        s += (double)C[a * nx + i] * w;
+                    }
+            } else if (ru) {                                   // (W_u r_u)_i
+                for (int b = 0; b < nu; ++b) s += (double)Wu[(i - nx) * nu + b] * (double)ru[k * nu + b];
+            }
+            qbar[q] = (T)s;
+        }
+    }
+}
+
 // Input of Alg. 1: hats = iterates (i_prev = i_cur), alpha_0 = 1, c^0 = c0.
 template <typename T>
 __global__ void k_begin(Prob<T> p)
@@ -426,6 +464,13 @@ Prob<T> make_prob(pimpc_s *h, double tol)
     p.lo = (const T *)h->lo; p.hi = (const T *)h->hi; p.dlo = (const T *)h->dlo; p.dhi = (const T *)h->dhi;
     p.bnd_stride = h->bnd_per_instance ? h->nb : 0;
     p.dbnd_stride = h->bnd_per_instance ? h->nu : 0;
+    p.lo_k = h->has_lok ? (const T *)h->lo_k : nullptr; p.hi_k = h->has_lok ? (const T *)h->hi_k : nullptr;
+    p.qbar_k = h->has_qbk ? (const T *)h->qbar_k : nullptr;
+    p.lok_bstride = h->lok_per_instance ? (size_t)h->N * h->nb : 0;
+    p.qbk_bstride = h->qbk_per_instance ? (size_t)h->N * h->nb : 0;
+    p.set_kind = h->set_kind; p.set_i0 = h->set_i0; p.set_len = h->set_len;
+    p.set_a = (const T *)h->set_a; p.set_b = h->set_b; p.set_inv_aa = h->set_inv_aa;
+    if (h->has_qbk) p.has_q = 1;
     p.H = (T *)h->H; p.M = (T *)h->M; p.S = (T *)h->S;
     p.buf_stride = (size_t)h->batch * h->N * h->rec;
     p.X = (T *)h->X; p.DU = (T *)h->DU;
@@ -468,6 +513,20 @@ static int setup_t(pimpc_s *h, const int *list, int nlist)
 int launch_setup(pimpc_s *h, const int *list_dev, int nlist)
 {
     return h->dtype == PIMPC_F64 ? setup_t<double>(h, list_dev, nlist) : setup_t<float>(h, list_dev, nlist);
+}
+
+int launch_tracking(pimpc_s *h, int ny, const void *C, const void *Wy, const void *Wu, const void *ry, const void *ru,
+                    int nref, void *qbar_out)
+{
+    const int total = h->nx * h->nx + h->nu * h->nu + nref * h->nb, th = 128, bl = std::min(1024, (total + th - 1) / th);
+    if (h->dtype == PIMPC_F64)
+        k_tracking<double><<<bl, th, 0, h->stream>>>(h->nx, h->nu, ny, (const double *)C, (const double *)Wy, (const double *)Wu,
+                                                     (const double *)ry, (const double *)ru, nref, (double *)h->Q, (double *)h->R, (double *)qbar_out);
+    else
+        k_tracking<float><<<bl, th, 0, h->stream>>>(h->nx, h->nu, ny, (const float *)C, (const float *)Wy, (const float *)Wu,
+                                                    (const float *)ry, (const float *)ru, nref, (float *)h->Q, (float *)h->R, (float *)qbar_out);
+    PIMPC_CUDA_TRY(h, cudaGetLastError());
+    return 1;
 }
 
 int launch_begin(pimpc_s *h)

@@ -98,13 +98,12 @@ __global__ void k_primal(Prob<T> p, StagedScratch<T> s, int spb)
     const size_t sk = (size_t)b * p.N + k;
     const T *Hk = p.H + sk * nb * nb;
     const T *hat = s.hat + p.st(b, k);
-    const T *qb = p.qbar + (size_t)b * p.qbar_stride;
     const T rho = (T)p.rho;
     const bool inner = (k < p.N - 1);
     const T *g1 = s.G + (sk + (inner ? 1 : 0)) * nb;
     T x = (T)0;
     for (int j = 0; j < nb; ++j) {
-        T h = qb[j] + rho * (hat[p.oZ() + j] - hat[p.oTH() + j]);
+        T h = p.qbar_at(b, k, j) + rho * (hat[p.oZ() + j] - hat[p.oTH() + j]);
         if (inner) h += rho * g1[j];
         x += Hk[j * nb + i] * h;            // H symmetric: column i == row i, coalesced over i
     }
@@ -125,6 +124,8 @@ template <typename T>
 __global__ void k_dual(Prob<T> p, StagedScratch<T> s, int spb)
 {
     __shared__ double red[32];
+    extern __shared__ __align__(16) unsigned char cand_raw[];  // [spb][nb] arguments of Proj (only with a general set)
+    T *cand = reinterpret_cast<T *>(cand_raw);
     const int b = blockIdx.y;
     const InstCtl c = p.ctl[b];
     if (c.done) return;
@@ -132,14 +133,15 @@ __global__ void k_dual(Prob<T> p, StagedScratch<T> s, int spb)
     const int t = threadIdx.x, ks = t / nb, i = t - ks * nb;
     const int k = blockIdx.x * spb + ks;
     T acc = (T)0;
-    if (ks < spb && k < p.N) {
+    const bool act = ks < spb && k < p.N;
+    const bool gset = p.set_kind != PIMPC_SET_NONE;            // uniform over the grid
+    T av = (T)0, bv = (T)0, zarg = (T)0;
+    if (act) {
         const size_t sk = (size_t)b * p.N + k;
         const T *Ak = p.A + sk * nx * nx, *Bk = p.B + sk * nx * nu;
         const T *hat = s.hat + p.st(b, k);
         const T *du = p.DU + sk * nu;
-        T *nw = p.S + (size_t)c.i_new * p.buf_stride + p.st(b, k);
         // a = Bbar du + betahat ; b = Abar xbar_k + ebar - lambdahat, xbar_k = X[k-1] (new) or xbar_0
-        T av, bv;
         if (i < nx) {
             av = (T)0;
             for (int j = 0; j < nu; ++j) av += Bk[i * nu + j] * du[j];
@@ -157,14 +159,25 @@ __global__ void k_dual(Prob<T> p, StagedScratch<T> s, int spb)
             av = du[i - nx];
             bv = (k == 0) ? p.uprev[(size_t)b * nu + (i - nx)] : p.X[(sk - 1) * nb + i];
         }
+        av += hat[p.oBE() + i];
+        bv -= hat[p.oLA() + i];
+        zarg = ((T)2 * (p.X[sk * nb + i] + hat[p.oTH() + i] + bv) + (av - bv)) / (T)3;       // argument of Proj
+        if (gset) cand[ks * nb + i] = zarg;
+    }
+    if (gset) __syncthreads();
+    if (act) {
+        const size_t sk = (size_t)b * p.N + k;
+        const T *hat = s.hat + p.st(b, k);
+        const T *du = p.DU + sk * nu;
+        T *nw = p.S + (size_t)c.i_new * p.buf_stride + p.st(b, k);
         const T zh = hat[p.oZ() + i], vh = hat[p.oV() + i], thh = hat[p.oTH() + i];
         const T beh = hat[p.oBE() + i], lah = hat[p.oLA() + i];
-        av += beh;
-        bv -= lah;
         const T gam = av - bv;
         const T x = p.X[sk * nb + i];
-        const T lo = p.lo[(size_t)b * p.bnd_stride + i], hi = p.hi[(size_t)b * p.bnd_stride + i];
-        const T zn = clipT(((T)2 * (x + thh + bv) + gam) / (T)3, lo, hi);
+        // z_{k+1} = Proj_Xbar(.): the box on every component outside the general set, the set's closed form inside it
+        T zn;
+        if (gset && i >= p.set_i0 && i < p.set_i0 + p.set_len) zn = proj_set_component(p, cand + ks * nb + p.set_i0, i - p.set_i0);
+        else zn = clipT(zarg, p.lo_at(b, k, i), p.hi_at(b, k, i));
         const T vn = (T)0.5 * (zn + gam);
         const T thn = thh + x - zn;
         const T ben = av - vn;
@@ -263,7 +276,7 @@ int run_staged_t(pimpc_s *h, int iters, double tol)
         k_hat<T><<<grid, threads, 0, h->stream>>>(p, s, spb);
         k_adj<T><<<grid, threads, 0, h->stream>>>(p, s, spb);
         k_primal<T><<<grid, threads, 0, h->stream>>>(p, s, spb);
-        k_dual<T><<<grid, threads, 0, h->stream>>>(p, s, spb);
+        k_dual<T><<<grid, threads, h->set_kind ? (size_t)spb * nb * sizeof(T) : 0, h->stream>>>(p, s, spb);
         k_decide<T><<<dgrid, dth, 0, h->stream>>>(p, it);
     }
     PIMPC_CUDA_TRY(h, cudaGetLastError());

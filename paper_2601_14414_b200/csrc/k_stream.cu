@@ -176,7 +176,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
     const long long s0 = cta * S_tot / G, s1 = (cta + 1) * S_tot / G;
     const int b_first = (int)(s0 / N1), n_local = (int)((s1 - 1) / N1) - b_first + 1;
     const T rho = (T)p.rho;
-    const bool has_du = p.has_du != 0, has_q = p.has_q != 0;
+    const bool has_du = p.has_du != 0, has_q = p.has_q != 0, gset = p.set_kind != PIMPC_SET_NONE;
     const int ci = tid % IP, prt = tid / IP;              // column index / row-range part of the column products
     const int di = tid - 4 * NX;                           // component of the dual update (threads >= 4 NX)
 
@@ -337,7 +337,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         if (i >= NX) g += wv[i];                                    // the [0 I] rows of Abar_{j+1}
                         h += rho * g;
                     }
-                    if (has_q) h += p.qbar[(size_t)b * p.qbar_stride + i];
+                    if (has_q) h += p.qbar_at(b, j, i);
                     hv[i] = h; hv[i + NB] = h;
                 }
                 if (tid >= IP && tid < IP + NU && do_next) {
@@ -409,18 +409,30 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         avc[pn * IP + r] = s1_ + hs[3 * NB + r];                   // a = Bbar du + betahat
                     }
                 }
-                if (di >= 0 && di < NB) {
+                const bool dthread = di >= 0 && di < NB;
+                if (dthread && do_next && di >= NX) {
+                    bc[pn * IP + di] = xv[di] - hs[4 * NB + di];
+                    avc[pn * IP + di] = duc[pn * IP + di - NX] + hs[3 * NB + di];
+                }
+                // argument of Proj of stage j (Thm 1, proof form, R1); with a general set (pimpc_set_constraint) the whole
+                // vector is staged in shared memory first (xp is free after phase E) -- a CTA-uniform extra barrier
+                T zarg = (T)0;
+                if (dthread && do_dual) {
                     const int i = di;
-                    if (do_next && i >= NX) {
-                        bc[pn * IP + i] = xv[i] - hs[4 * NB + i];
-                        avc[pn * IP + i] = duc[pn * IP + i - NX] + hs[3 * NB + i];
-                    }
+                    const T av = avc[pj * IP + i], bv = bc[pj * IP + i];
+                    zarg = ((T)2 * (xv[i] + hj[2 * NB + i] + bv) + (av - bv)) * (T)(1.0 / 3.0);
+                    if (gset) xp[i] = zarg;
+                }
+                if (gset && do_dual) __syncthreads();
+                if (dthread) {
+                    const int i = di;
                     if (do_dual) {
                         const T zh = hj[i], vh = hj[NB + i], thh = hj[2 * NB + i], beh = hj[3 * NB + i], lah = hj[4 * NB + i];
                         const T av = avc[pj * IP + i], bv = bc[pj * IP + i], x = xv[i];
-                        const T lo = p.lo[(size_t)b * p.bnd_stride + i], hi = p.hi[(size_t)b * p.bnd_stride + i];
                         const T gam = av - bv;
-                        const T zn = clips(((T)2 * (x + thh + bv) + gam) * (T)(1.0 / 3.0), lo, hi);   // Thm 1 (proof form, R1)
+                        T zn;
+                        if (gset && i >= p.set_i0 && i < p.set_i0 + p.set_len) zn = proj_set_component(p, xp + p.set_i0, i - p.set_i0);
+                        else zn = clips(zarg, p.lo_at(b, j, i), p.hi_at(b, j, i));
                         const T vn = (T)0.5 * (zn + gam);
                         const T thn = thh + x - zn, ben = av - vn, lan = zn - bv - vn;
                         const T d0 = thn - thh, d1 = ben - beh, d2 = lan - lah, d3 = zn - zh, d4 = vn - vh;

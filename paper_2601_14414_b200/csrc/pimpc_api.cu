@@ -323,7 +323,7 @@ int pimpc_destroy(pimpc_t h)
     void *ptrs[] = {h->A, h->B, h->e, h->x0, h->uprev, h->Q, h->R, h->P, h->Wdu, h->qbar, h->lo, h->hi, h->dlo, h->dhi,
                     h->H, h->M, h->S, h->X, h->DU, h->ctl, h->partial, h->hist_c, h->hist_a, h->err,
                     h->hat, h->W, h->G, h->rhs, h->blob, h->alpha_tab, h->kappa_tab, h->spartial, h->coop_buf, h->stage_buf,
-                    h->dirty_dev, h->res_part};
+                    h->dirty_dev, h->res_part, h->lo_k, h->hi_k, h->qbar_k, h->set_a, h->trk};
     for (void *p : ptrs)                         // memory carved from the caller's workspace is the caller's
         if (p && !(h->ws && (unsigned char *)p >= h->ws && (unsigned char *)p < h->ws + h->ws_bytes)) cudaFree(p);
     for (auto &e : h->ev) if (e) cudaEventDestroy(e);
@@ -405,6 +405,7 @@ int pimpc_set_cost(pimpc_t h, const void *Q, const void *R, const void *P, const
     if (qbar) { rc = copy_in(h, h->qbar, qbar, rep * h->nb * esz); if (rc) return rc; }
     else PIMPC_CUDA_TRY(h, cudaMemsetAsync(h->qbar, 0, (size_t)h->batch * h->nb * esz, h->stream));
     h->has_P = P != nullptr; h->has_wdu = Wdu != nullptr; h->has_q = qbar != nullptr;
+    h->has_qbk = 0;                                       // a per-stage linear term of an earlier call is replaced too
     h->cost_per_instance = per_instance ? 1 : 0;
     h->cache_dirty = true;
     return PIMPC_OK;
@@ -441,6 +442,97 @@ int pimpc_set_bounds(pimpc_t h, const void *lo, const void *hi, const void *du_l
     }
     if (had_du != h->has_du) h->cache_dirty = true;       // M_k contains the +I of the du block (R12)
     h->bnd_per_instance = per_instance ? 1 : 0;
+    return PIMPC_OK;
+}
+
+int pimpc_set_tracking(pimpc_t h, int ny, const void *C, const void *Wy, const void *Wu, const void *ry, const void *ru,
+                       int per_stage)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    DeviceGuard guard(h);
+    if (ny <= 0 || ny > PIMPC_MAX_NB || !C || !Wy || !Wu) return fail(h, PIMPC_EINVAL, "set_tracking: ny, C, Wy, Wu are required");
+    if (h->cost_per_instance) return fail(h, PIMPC_EINVAL, "set_tracking: a per-instance cost is set; use pimpc_set_cost");
+    const size_t esz = h->esz, nref = per_stage ? h->N : 1;
+    const size_t bC = (size_t)ny * h->nx * esz, bWy = (size_t)ny * ny * esz, bWu = (size_t)h->nu * h->nu * esz;
+    const size_t bry = nref * ny * esz, bru = nref * h->nu * esz;
+    auto al = [](size_t v) { return (v + 255) / 256 * 256; };
+    rc = pimpc_grow(h, &h->trk, &h->trk_cap, al(bC) + al(bWy) + al(bWu) + al(bry) + al(bru)); if (rc) return rc;
+    unsigned char *base = (unsigned char *)h->trk;
+    void *dC = base, *dWy = base + al(bC), *dWu = (unsigned char *)dWy + al(bWy);
+    void *dry = (unsigned char *)dWu + al(bWu), *dru = (unsigned char *)dry + al(bry);
+    rc = copy_in(h, dC, C, bC); if (rc) return rc;
+    rc = copy_in(h, dWy, Wy, bWy); if (rc) return rc;
+    rc = copy_in(h, dWu, Wu, bWu); if (rc) return rc;
+    if (ry) { rc = copy_in(h, dry, ry, bry); if (rc) return rc; }
+    if (ru) { rc = copy_in(h, dru, ru, bru); if (rc) return rc; }
+    void *qout = h->qbar;
+    if (per_stage) {
+        rc = pimpc_grow(h, &h->qbar_k, &h->qbk_cap, (size_t)h->N * h->nb * esz); if (rc) return rc;
+        qout = h->qbar_k;
+    }
+    const int n = launch_tracking(h, ny, dC, dWy, dWu, ry ? dry : nullptr, ru ? dru : nullptr, (int)nref, qout);
+    if (n < 0) return n;
+    h->info.total_launches += n;
+    h->has_P = 0; h->has_q = 1;
+    h->has_qbk = per_stage ? 1 : 0; h->qbk_per_instance = 0;
+    if (per_stage) h->blob_dirty = true;
+    h->cache_dirty = true;
+    return PIMPC_OK;
+}
+
+int pimpc_set_stage_terms(pimpc_t h, const void *lo, const void *hi, const void *qbar, int per_instance)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    DeviceGuard guard(h);
+    if ((lo == nullptr) != (hi == nullptr)) return fail(h, PIMPC_EINVAL, "set_stage_terms: lo and hi must be given together");
+    const size_t rep = per_instance ? h->batch : 1, n = rep * h->N * h->nb, bytes = n * h->esz;
+    if (lo) {
+        std::vector<double> a, b;
+        rc = fetch_host(h, lo, n, a); if (rc) return rc;
+        rc = fetch_host(h, hi, n, b); if (rc) return rc;
+        for (size_t i = 0; i < n; ++i)
+            if (std::isnan(a[i]) || std::isnan(b[i]) || a[i] > b[i]) return fail(h, PIMPC_EINVAL, "stage bounds: lo > hi or NaN");
+        rc = pimpc_grow(h, &h->lo_k, &h->lok_cap, bytes); if (rc) return rc;
+        rc = pimpc_grow(h, &h->hi_k, &h->hik_cap, bytes); if (rc) return rc;
+        rc = copy_in(h, h->lo_k, lo, bytes); if (rc) return rc;
+        rc = copy_in(h, h->hi_k, hi, bytes); if (rc) return rc;
+    }
+    h->has_lok = lo != nullptr; h->lok_per_instance = per_instance ? 1 : 0;
+    if (qbar) {
+        rc = pimpc_grow(h, &h->qbar_k, &h->qbk_cap, bytes); if (rc) return rc;
+        rc = copy_in(h, h->qbar_k, qbar, bytes); if (rc) return rc;
+    }
+    h->has_qbk = qbar != nullptr; h->qbk_per_instance = per_instance ? 1 : 0;
+    return PIMPC_OK;
+}
+
+int pimpc_set_constraint(pimpc_t h, int kind, int i0, int len, const void *a, double b)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    DeviceGuard guard(h);
+    if (kind == PIMPC_SET_NONE) { h->set_kind = PIMPC_SET_NONE; return PIMPC_OK; }
+    if (kind < PIMPC_SET_NONE || kind > PIMPC_SET_L1BALL) return fail(h, PIMPC_EINVAL, "set_constraint: bad kind");
+    if (i0 < 0 || len <= 0 || i0 + len > h->nb) return fail(h, PIMPC_EINVAL, "set_constraint: component range out of [0, nx + nu)");
+    if (!std::isfinite(b)) return fail(h, PIMPC_EINVAL, "set_constraint: b is not finite");
+    const bool lin = kind == PIMPC_SET_HALFSPACE || kind == PIMPC_SET_HYPERPLANE;
+    if (kind == PIMPC_SET_SOC && len < 2) return fail(h, PIMPC_EINVAL, "set_constraint: a second-order cone needs len >= 2");
+    if (kind == PIMPC_SET_L1BALL && b < 0.0) return fail(h, PIMPC_EINVAL, "set_constraint: negative radius");
+    double inv_aa = 0.0;
+    if (lin) {
+        if (!a) return fail(h, PIMPC_EINVAL, "set_constraint: a is required for a halfspace / hyperplane");
+        std::vector<double> v;
+        rc = fetch_host(h, a, (size_t)len, v); if (rc) return rc;
+        double aa = 0.0;
+        for (double x : v) { if (!std::isfinite(x)) return fail(h, PIMPC_EINVAL, "set_constraint: a is not finite"); aa += x * x; }
+        if (!(aa > 0.0)) return fail(h, PIMPC_EINVAL, "set_constraint: a is zero");
+        inv_aa = 1.0 / aa;
+        rc = pimpc_grow(h, &h->set_a, &h->set_a_cap, (size_t)len * h->esz); if (rc) return rc;
+        rc = copy_in(h, h->set_a, a, (size_t)len * h->esz); if (rc) return rc;
+    }
+    h->set_kind = kind; h->set_i0 = i0; h->set_len = len; h->set_b = b; h->set_inv_aa = inv_aa;
     return PIMPC_OK;
 }
 
@@ -491,6 +583,12 @@ int pimpc_solve(pimpc_t h, int max_iters, double tol)
 
     int engine = h->engine_req;
     std::string why;
+    // per-stage boxes / linear terms and a general convex set are implemented by the STAGED and STREAM engines
+    const bool ext = has_stage_terms(h);
+    if (ext && (engine == PIMPC_ENGINE_RESIDENT || engine == PIMPC_ENGINE_COOP))
+        return fail(h, PIMPC_EINVAL, "per-stage terms / a general set need the STREAM or STAGED engine");
+    if (engine == PIMPC_ENGINE_AUTO && ext)
+        engine = stream_supported(h, &why) ? PIMPC_ENGINE_STREAM : PIMPC_ENGINE_STAGED;
     if (engine == PIMPC_ENGINE_AUTO)
         engine = resident_supported(h, &why) ? PIMPC_ENGINE_RESIDENT
                  : coop_supported(h, &why) ? PIMPC_ENGINE_COOP

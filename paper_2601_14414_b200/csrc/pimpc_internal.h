@@ -37,6 +37,14 @@ struct Prob {
     int cost_stride_q, cost_stride_r, qbar_stride;
     const T *lo, *hi, *dlo, *dhi;    // bounds; strides 0 = shared
     int bnd_stride, dbnd_stride;
+    // per-stage boxes / linear terms (pimpc_set_stage_terms, pimpc_set_tracking with per-stage references) or null;
+    // element (b, k, i) at [b * *_bstride + k * nb + i]
+    const T *lo_k, *hi_k, *qbar_k;
+    size_t lok_bstride, qbk_bstride;
+    // general convex set on the components [set_i0, set_i0 + set_len) of z (pimpc_set_constraint); set_kind = PIMPC_SET_*
+    int set_kind, set_i0, set_len;
+    const T *set_a;                  // [set_len] normal vector (halfspace, hyperplane)
+    double set_b, set_inv_aa;        // offset / radius; 1 / ||a||^2
     T *H, *M;                        // cache: [batch][N][nb][nb] (symmetric), [batch][N][nu][nu]
     T *S;                            // 3 rotating buffers of [batch][N][rec]
     size_t buf_stride;               // elements between buffers
@@ -58,7 +66,53 @@ struct Prob {
     __host__ __device__ int oLA() const { return 4 * nb; }
     __host__ __device__ int oD() const { return 5 * nb; }
     __host__ __device__ int oDE() const { return 5 * nb + nu; }
+    // box and linear term of row i of stage k of instance b
+    __device__ T lo_at(int b, int k, int i) const { return lo_k ? lo_k[(size_t)b * lok_bstride + (size_t)k * nb + i] : lo[(size_t)b * bnd_stride + i]; }
+    __device__ T hi_at(int b, int k, int i) const { return hi_k ? hi_k[(size_t)b * lok_bstride + (size_t)k * nb + i] : hi[(size_t)b * bnd_stride + i]; }
+    __device__ T qbar_at(int b, int k, int i) const { return qbar_k ? qbar_k[(size_t)b * qbk_bstride + (size_t)k * nb + i] : qbar[(size_t)b * qbar_stride + i]; }
 };
+
+// Projection of the candidate vector t[0..len) (shared or global memory, read by every calling thread) onto the general
+// set of the handle (closed forms of [22, Ch. 6]): returns component j of the projection.  Every thread
+// evaluates the few scalars the closed form needs redundantly, in the same fixed order (deterministic, no atomics).
+template <typename T>
+__device__ inline T proj_set_component(const Prob<T> &p, const T *t, int j)
+{
+    const int n = p.set_len;
+    const T tj = t[j];
+    if (p.set_kind == PIMPC_SET_HALFSPACE || p.set_kind == PIMPC_SET_HYPERPLANE) {
+        T at = (T)0;
+        for (int i = 0; i < n; ++i) at += p.set_a[i] * t[i];
+        T s = (at - (T)p.set_b) * (T)p.set_inv_aa;
+        if (p.set_kind == PIMPC_SET_HALFSPACE && !(at > (T)p.set_b)) s = (T)0;
+        return tj - s * p.set_a[j];
+    }
+    if (p.set_kind == PIMPC_SET_SOC) {                     // (x, r): inside -> t; ||x|| <= -r -> 0; else ((||x|| + r)/2)(x/||x||, 1)
+        T n2 = (T)0;
+        for (int i = 0; i < n - 1; ++i) n2 += t[i] * t[i];
+        const T nx_ = sqrt(n2), r = t[n - 1];
+        if (nx_ <= r) return tj;
+        if (nx_ <= -r) return (T)0;
+        const T s = (T)0.5 * (nx_ + r);
+        return j == n - 1 ? s : s * tj / nx_;
+    }
+    if (p.set_kind == PIMPC_SET_L1BALL) {                  // soft threshold with tau = max_m (sum of the m largest |t| - r) / m
+        T l1 = (T)0;
+        for (int i = 0; i < n; ++i) l1 += fabs(t[i]);
+        if (l1 <= (T)p.set_b) return tj;
+        T tau = (T)0;
+        for (int m = 0; m < n; ++m) {                      // candidate: the elements not smaller than |t_m|
+            const T um = fabs(t[m]);
+            T sum = (T)0; int cnt = 0;
+            for (int i = 0; i < n; ++i) { const T ui = fabs(t[i]); if (ui >= um) { sum += ui; ++cnt; } }
+            const T cand = (sum - (T)p.set_b) / (T)cnt;
+            tau = cand > tau ? cand : tau;
+        }
+        const T mag = fabs(tj) - tau;
+        return mag > (T)0 ? (tj > (T)0 ? mag : -mag) : (T)0;
+    }
+    return tj;
+}
 
 struct pimpc_s {
     int nx = 0, nu = 0, nb = 0, N = 0, batch = 0, rec = 0;
@@ -81,6 +135,15 @@ struct pimpc_s {
     void *lo = nullptr, *hi = nullptr, *dlo = nullptr, *dhi = nullptr;
     int bnd_per_instance = 0;
     int has_du = 0, has_e = 0, has_P = 0, has_wdu = 0, has_q = 0;
+    void *lo_k = nullptr, *hi_k = nullptr, *qbar_k = nullptr;   // per-stage boxes / linear terms, [batch or 1][N][nb]
+    size_t lok_cap = 0, hik_cap = 0, qbk_cap = 0;               // allocated bytes
+    int has_lok = 0, has_qbk = 0, lok_per_instance = 0, qbk_per_instance = 0;
+    int set_kind = 0, set_i0 = 0, set_len = 0;                  // general convex set (pimpc_set_constraint)
+    void *set_a = nullptr;
+    size_t set_a_cap = 0;
+    double set_b = 0.0, set_inv_aa = 0.0;
+    void *trk = nullptr;                                        // staging of pimpc_set_tracking's inputs
+    size_t trk_cap = 0;
     void *H = nullptr, *M = nullptr, *S = nullptr, *X = nullptr, *DU = nullptr;
     InstCtl *ctl = nullptr;
     double *partial = nullptr;
@@ -127,6 +190,8 @@ int launch_begin(pimpc_s *h);                       // Alg. 1 input: alpha=1, c_
 int run_staged(pimpc_s *h, int iters, double tol);  // v0 engine
 int run_resident(pimpc_s *h, int iters, double tol);
 bool resident_supported(const pimpc_s *h, std::string *why);
+bool resident2_plan(const pimpc_s *h, int *nxp, int *nup, int *maxn);   // padded shape of the two-rows-per-lane kernel
+int run_resident2(pimpc_s *h, int iters, double tol);
 int ensure_alpha_table(pimpc_s *h, int iters);     // alpha_j / kappa_j tables cover `iters` accepted steps; returns launches
 int run_coop(pimpc_s *h, int iters, double tol);
 bool coop_supported(const pimpc_s *h, std::string *why);
@@ -136,6 +201,12 @@ int launch_gather(pimpc_s *h, void *x, void *u, void *du, pimpc_result *res_dev)
 int launch_state_io(pimpc_s *h, int which, void *buf_dev, int set);
 int launch_zero_state(pimpc_s *h);
 int launch_shift(pimpc_s *h, int steps);              // warm-start shift of the current iterate (reading R18)
+// Q = C'W_y C, R = W_u, qbar[k] = (C'W_y r_y[k]; W_u r_u[k]) from the staged inputs (device, element type of the handle)
+int launch_tracking(pimpc_s *h, int ny, const void *C, const void *Wy, const void *Wu, const void *ry, const void *ru,
+                    int nref, void *qbar_out);
+inline bool has_stage_terms(const pimpc_s *h);
+
+inline bool has_stage_terms(const pimpc_s *h) { return h->has_lok || h->has_qbk || h->set_kind != 0; }
 
 // (Re)allocate an engine-private device buffer of at least `bytes` (kept if large enough); accounts device_bytes; a failed
 // cudaMalloc returns PIMPC_ENOMEM without poisoning the handle.

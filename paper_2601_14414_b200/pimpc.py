@@ -24,6 +24,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENOTPD = 0, -1, -2, -3, -4, -5
 F64, F32 = 0, 1
 ENGINE_AUTO, ENGINE_STAGED, ENGINE_RESIDENT, ENGINE_STREAM, ENGINE_COOP = 0, 1, 2, 3, 4
 ENGINES = {"auto": 0, "staged": 1, "resident": 2, "stream": 3, "coop": 4}
+SETS = {"none": 0, "halfspace": 1, "hyperplane": 2, "soc": 3, "l1ball": 4}
 X, Z, V, TH, BE, LA, D, DE, DU = range(9)
 STATE = {"X": X, "Z": Z, "V": V, "TH": TH, "BE": BE, "LA": LA, "D": D, "DE": DE, "DU": DU}
 
@@ -75,6 +76,9 @@ SYMBOLS = {
     "pimpc_set_stages": (_i, [_vp, _vp, _vp, _vp]),
     "pimpc_set_cost": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _i]),
     "pimpc_set_bounds": (_i, [_vp, _vp, _vp, _vp, _vp, _i]),
+    "pimpc_set_tracking": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp, _i]),
+    "pimpc_set_stage_terms": (_i, [_vp, _vp, _vp, _vp, _i]),
+    "pimpc_set_constraint": (_i, [_vp, _i, _i, _i, _vp, _d]),
     "pimpc_set_x0": (_i, [_vp, _vp, _vp]),
     "pimpc_solve": (_i, [_vp, _i, _d]),
     "pimpc_get": (_i, [_vp, _vp, _vp, _vp, _vp]),
@@ -210,6 +214,23 @@ class Solver:
         a = [self._in(v) for v in (lo, hi, du_lo, du_hi)]
         self._ck(self.lib.pimpc_set_bounds(self.h, *[_ptr(v) for v in a], int(per_instance)))
 
+    def set_tracking(self, C, Wy, Wu, ry=None, ru=None, per_stage=False):
+        C = self._in(C); ny = C.shape[0]
+        Wy = self._in(Wy, (ny, ny)); Wu = self._in(Wu, (self.nu, self.nu))
+        ry = self._in(ry, (self.N, ny) if per_stage else (ny,)); ru = self._in(ru, (self.N, self.nu) if per_stage else (self.nu,))
+        self._ck(self.lib.pimpc_set_tracking(self.h, int(ny), _ptr(C), _ptr(Wy), _ptr(Wu), _ptr(ry), _ptr(ru), int(per_stage)))
+
+    def set_stage_terms(self, lo=None, hi=None, qbar=None, per_instance=False):
+        a = [self._in(v) for v in (lo, hi, qbar)]
+        self._ck(self.lib.pimpc_set_stage_terms(self.h, *[_ptr(v) for v in a], int(per_instance)))
+
+    def set_constraint(self, kind, i0=0, length=0, a=None, b=0.0):
+        a = self._in(a)
+        if a is not None:
+            length = int(np.asarray(a).size) if not (torch is not None and isinstance(a, torch.Tensor)) else a.numel()
+        self._ck(self.lib.pimpc_set_constraint(self.h, SETS[kind] if isinstance(kind, str) else int(kind), int(i0), int(length),
+                                               _ptr(a), float(b if b is not None else 0.0)))
+
     def set_x0(self, x0, u_prev=None):
         x0 = self._in(x0, (self.batch, self.nx)); u_prev = self._in(u_prev, (self.batch, self.nu))
         self._ck(self.lib.pimpc_set_x0(self.h, _ptr(x0), _ptr(u_prev)))
@@ -220,6 +241,16 @@ class Solver:
         self.set_cost(p.Q, p.R, p.P, p.Wdu, p.qbar)
         self.set_bounds(p.lo, p.hi, p.du_lo, p.du_hi)
         self.set_x0(p.x0, p.u_prev)
+        lo_k, hi_k, qbar_k, cset = (getattr(p, n, None) for n in ("lo_k", "hi_k", "qbar_k", "cset"))
+        self.set_stage_terms(lo_k, hi_k, qbar_k)
+        if cset is None:
+            self.set_constraint("none")
+        else:
+            kind, i0, a, b = cset
+            if isinstance(a, (int, np.integer)):
+                self.set_constraint(kind, i0, int(a), None, b)
+            else:
+                self.set_constraint(kind, i0, 0, a, b)
 
     # ---- solve / results -------------------------------------------------------------------
     def solve(self, max_iters, tol=0.0):

@@ -44,6 +44,12 @@ class Problem:
     tol: float = 0.0
     dtypes: tuple = ("f64",)
     meta: dict = field(default_factory=dict)
+    # SURVEY 8(f) row 2 (all shared by the instances): general set (kind, i0, a or length, b) on part of (x_{k+1}; u_k),
+    # per-stage boxes [N][nb], per-stage linear terms [N][nb]
+    cset: tuple | None = None
+    lo_k: np.ndarray | None = None
+    hi_k: np.ndarray | None = None
+    qbar_k: np.ndarray | None = None
 
     @property
     def nb(self) -> int:
@@ -51,10 +57,14 @@ class Problem:
 
     def instance(self, b: int) -> dict:
         """Keyword arguments of one instance, in the naming both solvers' Python wrappers use."""
-        return dict(A=self.A[b], B=self.B[b], Q=self.Q, R=self.R, lo=self.lo, hi=self.hi, x0=self.x0[b],
-                    e=None if self.e is None else self.e[b], P=self.P, Wdu=self.Wdu, qbar=self.qbar,
-                    du_lo=self.du_lo, du_hi=self.du_hi,
-                    u_prev=None if self.u_prev is None else self.u_prev[b], rho=self.rho)
+        kw = dict(A=self.A[b], B=self.B[b], Q=self.Q, R=self.R, lo=self.lo, hi=self.hi, x0=self.x0[b],
+                  e=None if self.e is None else self.e[b], P=self.P, Wdu=self.Wdu, qbar=self.qbar,
+                  du_lo=self.du_lo, du_hi=self.du_hi,
+                  u_prev=None if self.u_prev is None else self.u_prev[b], rho=self.rho)
+        for name in ("cset", "lo_k", "hi_k", "qbar_k"):
+            if getattr(self, name) is not None:
+                kw[name] = getattr(self, name)
+        return kw
 
     def rounded(self, dtype: str) -> "Problem":
         """The same problem with every input rounded to `dtype` and promoted back to float64
@@ -62,10 +72,14 @@ class Problem:
         if dtype == "f64":
             return self
         r = lambda a: None if a is None else np.asarray(a, np.float32).astype(np.float64)
+        cs = self.cset
+        if cs is not None:
+            cs = (cs[0], cs[1], cs[2] if isinstance(cs[2], (int, np.integer)) else r(cs[2]),
+                  None if cs[3] is None else float(np.float32(cs[3])))
         return Problem(self.name, self.nx, self.nu, self.N, self.batch, r(self.A), r(self.B), r(self.Q),
                        r(self.R), r(self.lo), r(self.hi), r(self.x0), r(self.e), r(self.P), r(self.Wdu),
                        r(self.qbar), r(self.du_lo), r(self.du_hi), r(self.u_prev), self.rho, self.iters,
-                       self.tol, self.dtypes, dict(self.meta))
+                       self.tol, self.dtypes, dict(self.meta), cs, r(self.lo_k), r(self.hi_k), r(self.qbar_k))
 
 
 # --------------------------------------------------------------------------------------------
@@ -274,6 +288,33 @@ def cstr_problem(x, u_prev, t0, N, *, rho=1.0, iters=1000, ref=None) -> Problem:
                    np.array(CSTR["lo"]), np.array(CSTR["hi"]), x[None, :].copy(), e=e[None], Wdu=np.array([[CSTR["Wdu"]]]),
                    qbar=qbar, u_prev=u[None, :].copy(), rho=rho, iters=iters, tol=0.0, dtypes=("f64", "f32"),
                    meta=dict(t0=t0))
+
+
+# --------------------------------------------------------------------------------------------
+# AFTI-16: the printed model, output matrix, constraints and weights
+# --------------------------------------------------------------------------------------------
+AFTI16 = dict(
+    Ac=((-0.0151, -60.5651, 0.0, -32.174), (-0.0001, -1.3411, 0.9929, 0.0), (0.00018, 43.2541, -0.86939, 0.0), (0.0, 0.0, 1.0, 0.0)),
+    Bc=((-2.516, -13.136), (-0.1689, -0.2514), (-17.251, -1.5766), (0.0, 0.0)),
+    C=((0.0, 1.0, 0.0, 0.0), (0.0, 0.0, 0.0, 1.0)), Ts=0.05, u_max=25.0, y_max=(0.5, 100.0), Wy=(100.0, 100.0), Wdu=(0.1, 0.1))
+
+
+def afti16(N: int = 5, batch: int = 1, *, ref: float = 10.0, rho: float = 10.0, iters: int = 300, seed: int = 0):
+    """The AFTI-16 tracking problem of PAPER.md:319-329 with the matrices as printed: y = C x, |u_i| <= 25, -0.5 <= y_1 <=
+    0.5, -100 <= y_2 <= 100, W_y = diag(100, 100), W_u = 0, W_du = diag(0.1, 0.1), N = 5.  The paper discretises with a
+    zero-order hold and does not print the reference signal or rho: forward Euler (T_s = 0.05 s) and a constant pitch
+    reference `ref` stand in.  Because C selects states, the output constraints are a box on x_2 and x_4.  Returns
+    (Problem, tracking) where tracking = dict(C, Wy, Wu, ry, ru) is what pimpc_set_tracking takes.  The Problem's Q, R are
+    zero placeholders: forming (Q, R, qbar) from the tracking data is the solvers' arithmetic, not the generator's."""
+    a = AFTI16
+    A1 = np.eye(4) + a["Ts"] * np.array(a["Ac"]); B1 = a["Ts"] * np.array(a["Bc"])
+    rng = np.random.default_rng([*SEED, 16, seed])
+    x0 = 0.05 * rng.uniform(-1.0, 1.0, size=(batch, 4))
+    C = np.array(a["C"]); Wy = np.diag(a["Wy"]); Wu = np.zeros((2, 2)); ry = np.array([0.0, ref])
+    lo = np.array([-np.inf, -a["y_max"][0], -np.inf, -a["y_max"][1], -a["u_max"], -a["u_max"]])
+    p = Problem("AFTI16", 4, 2, N, batch, np.tile(A1, (batch, N, 1, 1)), np.tile(B1, (batch, N, 1, 1)), np.zeros((4, 4)), Wu,
+                lo, -lo, x0, Wdu=np.diag(a["Wdu"]), rho=rho, iters=iters, tol=0.0, dtypes=("f64", "f32"))
+    return p, dict(C=C, Wy=Wy, Wu=Wu, ry=ry, ru=np.zeros(2))
 
 
 def pad_problem(p: Problem, nx2: int, nu2: int) -> Problem:

@@ -182,3 +182,78 @@ def active_set_bruteforce(A, B, Q, R, lo, hi, x0, e=None, P=None, Wdu=None, qbar
     U = best[0]
     X = np.stack([Phi[k] @ U + phi[k] for k in range(N)])
     return U.reshape(N, nu), X, best[1]
+
+
+# ------------------------------------------------------------------------------------------------
+# general convex sets and the tracking cost: plain definitions, solved by library routines
+# ------------------------------------------------------------------------------------------------
+def set_constraints(kind, i0, a, b, n):
+    """Inequality functions g(zeta) >= 0 (and equalities h(zeta) = 0) that DEFINE the set of PAPER.md:166 on the
+    components [i0, i0 + n) of a stage vector zeta = (x_{k+1}; u_k).  Returns (list of ineq, list of eq)."""
+    sl = slice(i0, i0 + n)
+    if kind == "halfspace":
+        return [lambda z: b - a @ z[sl]], []
+    if kind == "hyperplane":
+        return [], [lambda z: a @ z[sl] - b]
+    if kind == "soc":                                  # ||x||_2 <= r (its gradient exists everywhere but on the axis)
+        return [lambda z: z[sl][-1] - np.sqrt(np.sum(z[sl][:-1] ** 2) + 1e-300)], []
+    if kind == "l1ball":                               # ||x||_1 <= r: one halfspace per sign pattern
+        signs = [np.array(s) for s in itertools.product((-1.0, 1.0), repeat=n)]
+        return [(lambda z, s=s: b - s @ z[sl]) for s in signs], []
+    raise ValueError(kind)
+
+
+def slsqp_qp(A, B, Q, R, lo, hi, x0, *, e=None, P=None, Wdu=None, qbar=None, u_prev=None, cset=None,
+             lo_k=None, hi_k=None, qbar_k=None):
+    """QP (1) with boxes (shared or per stage), an optional general set on part of (x_{k+1}; u_k) at every stage and
+    optional per-stage linear terms, solved by scipy's SLSQP on the condensed problem in U.  Returns (x [N][nx], u [N][nu])."""
+    from scipy.optimize import minimize
+    N, nx, nu, e, P, Wdu, qbar, u_prev = _defaults(A, B, e, P, Q, Wdu, qbar, u_prev)
+    Hc, fc, Phi, phi, Dm, d0 = condensed(A, B, Q, R, x0, e, P, Wdu, np.zeros(nx + nu), u_prev)
+    qk = np.tile(qbar, (N, 1)) if qbar_k is None else np.asarray(qbar_k, float)
+    for k in range(N):                                 # linear terms: - qx_k' x_{k+1} - qu_k' u_k
+        fc = fc - Phi[k].T @ qk[k, :nx]
+        fc[k * nu:(k + 1) * nu] -= qk[k, nx:]
+    lo_s = np.tile(lo, (N, 1)) if lo_k is None else np.asarray(lo_k, float)
+    hi_s = np.tile(hi, (N, 1)) if hi_k is None else np.asarray(hi_k, float)
+
+    def stage(U, k):
+        return np.concatenate([Phi[k] @ U + phi[k], U[k * nu:(k + 1) * nu]])
+
+    cons = []
+    for k in range(N):
+        for i in range(nx + nu):
+            if np.isfinite(lo_s[k, i]):
+                cons.append({"type": "ineq", "fun": (lambda U, k=k, i=i: stage(U, k)[i] - lo_s[k, i])})
+            if np.isfinite(hi_s[k, i]):
+                cons.append({"type": "ineq", "fun": (lambda U, k=k, i=i: hi_s[k, i] - stage(U, k)[i])})
+        if cset is not None:
+            kind, i0, a, b = cset
+            n = a if isinstance(a, (int, np.integer)) else len(a)
+            ineq, eq = set_constraints(kind, i0, None if isinstance(a, (int, np.integer)) else np.asarray(a, float), b, n)
+            cons += [{"type": "ineq", "fun": (lambda U, k=k, g=g: g(stage(U, k)))} for g in ineq]
+            cons += [{"type": "eq", "fun": (lambda U, k=k, g=g: g(stage(U, k)))} for g in eq]
+    best = None
+    for start in (np.zeros(N * nu), 0.05 * np.ones(N * nu)):
+        r = minimize(lambda U: 0.5 * U @ Hc @ U + fc @ U, start, jac=lambda U: Hc @ U + fc, constraints=cons,
+                     method="SLSQP", options={"ftol": 1e-15, "maxiter": 2000})
+        if best is None or (r.success and r.fun < best.fun):
+            best = r
+    U = best.x
+    return np.stack([Phi[k] @ U + phi[k] for k in range(N)]), U.reshape(N, nu)
+
+
+def tracking_least_squares(A, B, C, Wy, Wu, ry, ru, x0, e=None):
+    """Unconstrained problem (1a)-(1b),(1d) as ONE linear least-squares problem in U:
+    min sum_k 1/2 ||L_y' (C x_{k+1} - r_y)||^2 + 1/2 ||L_u' (u_k - r_u)||^2,  W = L L'.  Never forms C'W_yC or qbar."""
+    N, nx, _ = A.shape
+    nu = B.shape[2]
+    _, _, Phi, phi, _, _ = condensed(A, B, np.eye(nx), np.eye(nu), x0, e)
+    Ly, Lu = np.linalg.cholesky(Wy), np.linalg.cholesky(Wu)
+    rows, rhs = [], []
+    for k in range(N):
+        rows.append(Ly.T @ C @ Phi[k]); rhs.append(Ly.T @ (ry - C @ phi[k]))
+        sel = np.zeros((nu, N * nu)); sel[:, k * nu:(k + 1) * nu] = np.eye(nu)
+        rows.append(Lu.T @ sel); rhs.append(Lu.T @ ru)
+    U = np.linalg.lstsq(np.vstack(rows), np.concatenate(rhs), rcond=None)[0]
+    return np.stack([Phi[k] @ U + phi[k] for k in range(N)]), U.reshape(N, nu)

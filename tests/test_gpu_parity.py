@@ -92,11 +92,11 @@ def test_config4_full_batch_every_instance(oracle, pimpc):
     parity.check_properties(p, "f32", g)
     with ThreadPoolExecutor(os.cpu_count() or 4) as ex:
         out = list(ex.map(lambda b: parity.check_instance(oracle, p, "f32", g, b, label="C4/f32/auto"), range(p.batch)))
-    nrep = sum(int(r) for _, r in out)
+    nrep = sum(int(r == 1) for _, r in out)
     st = parity.STATS["C4/f32/auto"]
     print(f"C4: worst {st['worst']:.2e}, c_rel {st['c_rel']:.2e}, replays {nrep} of {p.batch}, widest flip margin {st['flip_margin']}")
-    # fp32 c carries ~2-3e-7 relative error, so a few dozen of the 819 200 decisions are genuine near-ties
-    assert nrep <= 64
+    print(f"    band of the widest flip {st['flip_band']}")
+    assert nrep <= parity.replay_bound("f32", 200 * p.batch)
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
@@ -141,12 +141,14 @@ def test_stream_engine_all_options(oracle, pimpc, shape, grid, dtype):
 @pytest.mark.parametrize("shape", [(10, 3, 17, 2), (20, 6, 9, 2), (30, 10, 7, 1), (50, 15, 5, 2)])
 def test_stream_engine_paper_table1_shapes(oracle, pimpc, shape, grid, dtype):
     """The (n, m) of the paper's Table I, odd nb included (circulant storage of H without a
-    self-paired diagonal); AUTO must pick STREAM for them."""
+    self-paired diagonal); AUTO must pick a fused engine for them (the register-resident one for (10, 3) in fp32)."""
     nx, nu, N, batch = shape
     p = wl.random_ltv(nx, nu, N, batch, seed=nx * 7 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
                       qbar=True, bounds=0.8, du_bound=0.5)
-    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="auto", iters=100, tol=0.0, opts=_tune(grid=grid))
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="stream", iters=100, tol=0.0, opts=_tune(grid=grid))
     assert g["info"]["engine"] == pimpc.ENGINE_STREAM
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="auto", iters=100, tol=0.0)
+    assert g["info"]["engine"] != pimpc.ENGINE_STAGED         # a fused engine serves every Table-I shape up to (50, 15)
     parity.check_properties(p, dtype, g)
 
 
@@ -280,13 +282,14 @@ def test_shift_argument_validation_and_identity(pimpc):
 
 
 # ---- RESIDENT engine: every instantiation AUTO can reach ---------------------------------
-@pytest.mark.parametrize("N,batch,rows", [(57, 3, 0), (60, 2, 0), (64, 5, 0), (50, 3, 1), (23, 2, 1)])
+@pytest.mark.parametrize("N,batch,rows", [(57, 3, 0), (60, 2, 0), (64, 5, 0), (48, 3, 0), (49, 2, 0), (50, 3, 1), (23, 2, 1), (61, 2, 1)])
 def test_resident_fp32_quadrotor_one_row_per_lane(oracle, pimpc, N, batch, rows):
-    """fp32 (12, 4): horizons 57..64 run one row per lane (k_resident<float,12,4,1,800|1024>), as does any horizon with
-    tune.rows_per_lane = 1."""
+    """fp32 (12, 4): horizons 49..64 run k_res2 with G_k in shared memory (13..16 warps), tune.rows_per_lane = 1 the
+    one-row-per-lane kernel (k_resident<float,12,4,1,800|1024>)."""
     p = wl.quadrotor_ltv(N, batch, iters=150, tol=0.0)
     g, worst, nrep = parity.check(oracle, pimpc, p, "f32", engine="resident", opts=_tune(rows_per_lane=rows))
-    assert g["info"]["engine"] == pimpc.ENGINE_RESIDENT and g["info"]["block"] == 32 * ((N + 1) // 2)
+    assert g["info"]["engine"] == pimpc.ENGINE_RESIDENT
+    assert g["info"]["block"] == 32 * ((N + 1) // 2 if rows == 1 else (N + 3) // 4)
     parity.check_properties(p, "f32", g)
 
 
@@ -385,6 +388,112 @@ def test_large_shape_of_the_papers_table1(oracle, pimpc):
     """(n, m) = (100, 30), the largest shape of Table I: nb = 130 runs on the generic engines."""
     p = wl.paper_random(100, 30, 6, iters=40)
     g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="auto", iters=40, tol=0.0)
+
+
+# ---- SURVEY 8(f) row 2: general convex sets, per-stage terms, the tracking cost (PAPER.md:37, 166, 197) ----------
+SETS_GPU = {"halfspace": ("halfspace", 1, [1.0, 0.6, -0.8, 0.5], 0.1), "hyperplane": ("hyperplane", 2, [1.0, -2.0, 0.7], 0.05),
+            "soc": ("soc", 5, 3, None), "l1ball": ("l1ball", 5, 3, 0.35), "l1ball-wide": ("l1ball", 0, 8, 1.2)}
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("kind", list(SETS_GPU))
+@pytest.mark.parametrize("engine,grid", [("staged", 0), ("stream", 0), ("stream", 3), ("auto", 0)])
+def test_general_convex_sets(oracle, pimpc, engine, grid, kind, dtype):
+    """z_{k+1} = Proj onto box x {halfspace, hyperplane, second-order cone, l1 ball} (Thm 1), with
+    per-stage boxes on the other components and per-stage linear terms; (nx, nu) = (5, 3), N = 17, batch 2.  The set is
+    active (checked on the oracle's iterate: the projection moved at least one stage)."""
+    nx, nu, N, batch = 5, 3, 17, 2
+    p = wl.random_ltv(nx, nu, N, batch, seed=166, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5, scale=0.2)
+    rng = np.random.default_rng([2601, 14414, 8, 2])
+    p.cset = SETS_GPU[kind]
+    p.lo_k = -rng.uniform(0.3, 0.9, size=(N, nx + nu)); p.hi_k = rng.uniform(0.3, 0.9, size=(N, nx + nu))
+    p.qbar_k = 0.3 * rng.normal(size=(N, nx + nu))
+    if engine == "stream":
+        if (nx, nu) == (5, 3):                            # STREAM has no (5, 3) instantiation: the same test on (12, 4)
+            nx, nu = 12, 4
+            p = wl.random_ltv(nx, nu, N, batch, seed=166, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5, scale=0.2)
+            p.cset = SETS_GPU[kind]
+            p.lo_k = -rng.uniform(0.3, 0.9, size=(N, nx + nu)); p.hi_k = rng.uniform(0.3, 0.9, size=(N, nx + nu))
+            p.qbar_k = 0.3 * rng.normal(size=(N, nx + nu))
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine=engine, iters=150, tol=0.0, opts=_tune(grid=grid))
+    assert g["info"]["engine"] in (pimpc.ENGINE_STAGED, pimpc.ENGINE_STREAM)
+    k_, i0, a, b = p.cset
+    n = a if isinstance(a, int) else len(a)
+    Zs = g["Z"][..., i0:i0 + n].astype(np.float64)
+    if k_ == "halfspace":
+        val = Zs @ np.asarray(a); assert np.all(val <= b + 1e-5) and np.any(val >= b - 1e-5)
+    elif k_ == "hyperplane":
+        assert np.max(np.abs(Zs @ np.asarray(a) - b)) <= 1e-5
+    elif k_ == "soc":
+        gap = Zs[..., -1] - np.linalg.norm(Zs[..., :-1], axis=-1); assert np.all(gap >= -1e-5) and np.any(gap <= 1e-5)
+    else:
+        l1 = np.sum(np.abs(Zs), axis=-1); assert np.all(l1 <= b + 1e-5) and np.any(l1 >= b - 1e-5)
+    out = np.delete(g["Z"], np.arange(i0, i0 + n), axis=-1)
+    assert np.all(out >= np.delete(p.lo_k, np.arange(i0, i0 + n), axis=-1).astype(out.dtype))
+    assert np.all(out <= np.delete(p.hi_k, np.arange(i0, i0 + n), axis=-1).astype(out.dtype))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("engine", ["staged", "auto", "stream", "coop"])
+def test_tracking_entry_point_afti16(oracle, pimpc, engine, dtype):
+    """pimpc_set_tracking(C, W_y, W_u, r_y, r_u) forms Q = C'W_y C, R = W_u, qbar on the device; the
+    oracle forms them with its own routine.  Problem: the AFTI-16 model with its output constraints -0.5 <= y_1 <= 0.5
+    (PAPER.md:321-329), N = 5 as in the paper and N = 23."""
+    for N, batch in ((5, 3), (23, 1)):
+        if engine == "coop" and batch != 1:
+            continue
+        p, trk = wl.afti16(N, batch, iters=300)
+        pr = p.rounded(dtype)
+        r32 = (lambda a: np.asarray(a, np.float32).astype(np.float64)) if dtype == "f32" else (lambda a: a)
+        Q, R, qbar = oracle.tracking(r32(trk["C"]), r32(trk["Wy"]), r32(trk["Wu"]), r32(trk["ry"]), r32(trk["ru"]))
+        s = pimpc.Solver(4, 2, N, batch, dtype=dtype, engine=engine, rho=p.rho, history=300)
+        s.set_stages(p.A, p.B); s.set_bounds(p.lo, p.hi); s.set_x0(p.x0)
+        s.set_cost(np.eye(4), np.eye(2), None, p.Wdu)                    # Wdu stays; Q, R, qbar are replaced below
+        s.set_tracking(trk["C"], trk["Wy"], trk["Wu"], trk["ry"], trk["ru"])
+        s.solve(300)
+        c, acc = s.get_history()
+        for b in range(batch):
+            a = pr.instance(b); a.update(Q=Q, R=R, qbar=qbar)
+            o = oracle.solve(**a, max_iters=300, tol=0.0)
+            assert list(acc[b]) == list(o.acc_hist) or dtype == "f32"
+            if list(acc[b]) != list(o.acc_hist):
+                o = oracle.solve(**a, max_iters=300, tol=0.0, forced=acc[b])
+            for name in ("Z", "V", "TH", "X"):
+                assert parity.relerr(s.get_state(name)[b], getattr(o, name)) <= parity.TOL[dtype], (engine, N, name)
+        y1 = s.get_state("Z")[..., 1]
+        assert np.all(np.abs(y1) <= 0.5)
+        s.close()
+
+
+@pytest.mark.parametrize("engine", ["staged", "stream"])
+def test_tracking_with_time_varying_references(oracle, pimpc, engine):
+    """per_stage references r_y[k], r_u[k]: qbar differs per stage (STAGED / STREAM)."""
+    nx, nu, N = 12, 4, 21
+    p = wl.random_ltv(nx, nu, N, 2, seed=9, affine=True, u_prev=True, bounds=0.8, du_bound=0.5, scale=0.2)
+    rng = np.random.default_rng([2601, 14414, 197, 2])
+    C = rng.normal(size=(3, nx)); Wy = np.diag([2.0, 1.0, 0.5]); Wu = 0.1 * np.eye(nu)
+    ry = 0.3 * rng.normal(size=(N, 3)); ru = 0.05 * rng.normal(size=(N, nu))
+    s = pimpc.Solver(nx, nu, N, 2, dtype="f64", engine=engine, history=120)
+    s.set_problem(p)
+    s.set_tracking(C, Wy, Wu, ry, ru, per_stage=True)
+    s.solve(120)
+    qk = np.stack([oracle.tracking(C, Wy, Wu, ry[k], ru[k])[2] for k in range(N)])
+    Q, R, _ = oracle.tracking(C, Wy, Wu, None, None)
+    for b in range(2):
+        a = p.instance(b); a.update(Q=Q, R=R, qbar=None, P=None, qbar_k=qk)
+        o = oracle.solve(**a, max_iters=120, tol=0.0)
+        for name in ("Z", "V", "TH", "X"):
+            assert parity.relerr(s.get_state(name)[b], getattr(o, name)) <= 1e-9, (engine, name)
+
+
+def test_resident_pad_stages_with_a_box_that_excludes_zero(oracle, pimpc):
+    """A horizon that does not fill the last warp leaves pad stages in the CTA; they must stay exactly zero even when
+    the box excludes 0 (their constants are a block of zeros, not the instance's bounds)."""
+    for dtype, shape in (("f32", (12, 4, 50, 3)), ("f64", (4, 2, 9, 2)), ("f32", (4, 2, 61, 2))):
+        nx, nu, N, batch = shape
+        p = wl.random_ltv(nx, nu, N, batch, seed=77, affine=True, u_prev=True, bounds=0.9, du_bound=0.5, scale=0.2)
+        p.lo = p.lo.copy(); p.lo[1] = 0.15; p.lo[nx] = 0.1            # x_2 >= 0.15, u_1 >= 0.1
+        g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="resident", iters=120, tol=0.0)
 
 
 # ---- odd shapes, optional terms, edge cases -----------------------------------------------------

@@ -323,3 +323,138 @@ def test_shift_warm_start_definition_and_benefit(oracle):
     cold = oracle.solve(**kw, max_iters=2, tol=0.0)
     hot = oracle.solve(**kw, max_iters=2, tol=0.0, warm=warm)
     assert hot.c_hist[0] < 0.2 * cold.c_hist[0]           # 0.42 vs 4.1 on config 1 (short horizon: the tail is new)
+
+
+# ----------------------------------------------------------------------------------------------
+# the other projections of PAPER.md:166, per-stage data, the tracking cost (1a)
+# ----------------------------------------------------------------------------------------------
+def _feasible(kind, y, a, b, tol=0.0):
+    if kind == "halfspace":
+        return a @ y <= b + tol
+    if kind == "hyperplane":
+        return abs(a @ y - b) <= tol
+    if kind == "soc":
+        return np.linalg.norm(y[:-1]) <= y[-1] + tol
+    return np.sum(np.abs(y)) <= b + tol
+
+
+@pytest.mark.parametrize("kind,n", [("halfspace", 4), ("hyperplane", 3), ("soc", 4), ("l1ball", 5)])
+def test_projections_are_nearest_points(oracle, kind, n):
+    """Each projection against what DEFINES it (not its closed form): the result is feasible, a fixed point of the map,
+    satisfies the variational inequality <t - P t, y - P t> <= 0 for every feasible y (the optimality condition of the
+    nearest-point problem), and equals scipy's numerical minimiser of ||y - t||^2 over the set."""
+    from scipy.optimize import minimize
+    rng = np.random.default_rng([2601, 14414, 166, n])
+    a = rng.normal(size=n) if kind in ("halfspace", "hyperplane") else None
+    b = {"halfspace": 0.3, "hyperplane": -0.2, "soc": 0.0, "l1ball": 1.1}[kind]
+    moved = 0
+    for trial in range(30):
+        t = rng.normal(size=n) * (2.0 if trial % 3 else 0.3)
+        p = oracle.project(kind, t, a, b)
+        assert _feasible(kind, p, a, b, 1e-12)
+        np.testing.assert_allclose(oracle.project(kind, p, a, b), p, atol=1e-13)          # idempotent
+        moved += int(np.linalg.norm(p - t) > 1e-9)
+        ys = rng.normal(size=(400, n)) * 2.0                                              # feasible test points
+        if kind == "hyperplane":
+            ys = ys - np.outer((ys @ a - b) / (a @ a), a)
+        elif kind == "halfspace":
+            ys = ys - np.outer(np.maximum(ys @ a - b, 0.0) / (a @ a), a) - np.outer(rng.uniform(0, 1, 400), a)
+        elif kind == "soc":
+            ys[:, -1] = np.linalg.norm(ys[:, :-1], axis=1) + rng.uniform(0, 1, 400)
+        else:
+            ys = ys * (b * rng.uniform(0, 1, 400) / np.sum(np.abs(ys), axis=1))[:, None]
+        assert all(_feasible(kind, y, a, b, 1e-9) for y in ys)
+        assert np.max((ys - p) @ (t - p)) <= 1e-10
+        ineq, eq = ref.set_constraints(kind, 0, a, b, n)
+        cons = [{"type": "ineq", "fun": g} for g in ineq] + [{"type": "eq", "fun": g} for g in eq]
+        start = np.concatenate([np.zeros(n - 1), [1.0]]) if kind == "soc" else np.zeros(n)
+        r = minimize(lambda y: np.sum((y - t) ** 2), start, jac=lambda y: 2 * (y - t), constraints=cons,
+                     method="SLSQP", options={"ftol": 1e-16, "maxiter": 500})
+        np.testing.assert_allclose(p, r.x, atol=2e-6)
+    assert moved >= 10                                        # the set was really active
+    # hand-worked cases of [22, Ch. 6]
+    np.testing.assert_allclose(oracle.project("l1ball", [3.0, -1.0, 0.5], b=2.0), [2.0, 0.0, 0.0], atol=1e-15)
+    np.testing.assert_allclose(oracle.project("soc", [3.0, 4.0, 1.0]), [1.8, 2.4, 3.0], atol=1e-15)
+    np.testing.assert_allclose(oracle.project("soc", [3.0, 4.0, -6.0]), [0.0, 0.0, 0.0], atol=0)      # polar cone
+    np.testing.assert_allclose(oracle.project("soc", [3.0, 4.0, 6.0]), [3.0, 4.0, 6.0], atol=0)       # inside
+
+
+@pytest.mark.parametrize("cset", [("halfspace", 0, [1.0, 0.6, -0.8], -0.3), ("hyperplane", 1, [1.0, 2.0], 0.1),
+                                  ("soc", 2, 3, None), ("l1ball", 2, 3, 0.15), ("l1ball", 2, 2, 0.3)])
+def test_converged_solution_with_general_sets_matches_slsqp(oracle, cset):
+    """Theorem 1: the z-update is Proj of the same argument for ANY closed convex set.  The converged
+    oracle must reach the minimiser of QP (1) with that set on (x_{k+1}; u_k) -- computed here by scipy's SLSQP from the
+    set's defining inequalities, with the box still on the remaining components."""
+    kind, i0, a, b = cset
+    # the cone ||(u_1, u_2)||_2 <= u_3 and the l1 balls sit on the inputs, where they are always feasible
+    nu = a if isinstance(a, int) else 1
+    p = wl.random_ltv(2, nu, 4, 1, seed=166, affine=True, u_prev=True, bounds=None, du_bound=None, scale=0.2)
+    lo = np.concatenate([[-0.6, -0.6], -0.5 * np.ones(nu)]); hi = -lo
+    n = a if isinstance(a, int) else len(a)
+    for i in range(i0, i0 + n):                           # the set replaces the box on its components
+        lo[i], hi[i] = -np.inf, np.inf
+    if kind == "hyperplane" or (kind == "l1ball" and n == 2):      # keep the problem feasible: no state box
+        lo[:], hi[:] = -np.inf, np.inf
+    args = p.instance(0); args.update(lo=lo, hi=hi)
+    r = oracle.solve(**args, max_iters=60000, tol=1e-22, cset=cset)
+    assert r.c_last < 1e-22
+    xs, us = ref.slsqp_qp(p.A[0], p.B[0], p.Q, p.R, lo, hi, p.x0[0], e=p.e[0], u_prev=p.u_prev[0], cset=cset)
+    zs = np.hstack([xs, us])
+    ineq, eq = ref.set_constraints(kind, i0, None if isinstance(a, int) else np.asarray(a, float), b, n)
+    active = sum(int(min(abs(g(z)) for g in ineq + eq) < 1e-6) for z in zs)
+    assert active >= 1, "the test problem does not exercise the set"
+    np.testing.assert_allclose(r.x, xs, atol=2e-6)
+    np.testing.assert_allclose(r.u, us, atol=2e-6)
+    z = np.hstack([r.x, r.u])
+    assert all(g(zk) >= -1e-9 for zk in z for g in ineq) and all(abs(g(zk)) <= 1e-9 for zk in z for g in eq)
+
+
+def test_per_stage_boxes_and_linear_terms_match_slsqp(oracle):
+    """x_{k+1} in X_k, u_k in U_k and time-varying references (qbar_k): PAPER.md:37-47 with stage-dependent data."""
+    p = wl.random_ltv(2, 2, 5, 1, seed=37, affine=True, u_prev=True, bounds=None, du_bound=None, scale=0.2)
+    rng = np.random.default_rng([2601, 14414, 37])
+    hi_k = rng.uniform(0.15, 0.6, size=(5, 4)); lo_k = -rng.uniform(0.15, 0.6, size=(5, 4))
+    qbar_k = 0.5 * rng.normal(size=(5, 4))
+    r = oracle.solve(**p.instance(0), max_iters=60000, tol=1e-22, lo_k=lo_k, hi_k=hi_k, qbar_k=qbar_k)
+    assert r.c_last < 1e-22
+    xs, us = ref.slsqp_qp(p.A[0], p.B[0], p.Q, p.R, p.lo, p.hi, p.x0[0], e=p.e[0], u_prev=p.u_prev[0],
+                          lo_k=lo_k, hi_k=hi_k, qbar_k=qbar_k)
+    z = np.hstack([r.x, r.u])
+    assert np.sum(np.isclose(z, lo_k, atol=1e-9) | np.isclose(z, hi_k, atol=1e-9)) >= 3       # several stage bounds active
+    np.testing.assert_allclose(r.x, xs, atol=2e-6)
+    np.testing.assert_allclose(r.u, us, atol=2e-6)
+
+
+def test_tracking_cost_matches_least_squares_and_afti16_output_box(oracle):
+    """(1a) -> (Q, R, qbar) = (C'W_yC, W_u, col(C'W_y r_y, W_u r_u)): the converged unconstrained
+    iteration equals the least-squares solution of the tracking problem written with C, W_y, r_y, r_u directly.  Then the
+    AFTI-16 model as printed (forward Euler here, the paper uses a zero-order hold) with its output
+    constraint -0.5 <= y_1 <= 0.5, which is a box on x_2 because C selects states."""
+    rng = np.random.default_rng([2601, 14414, 197])
+    p = wl.random_ltv(3, 2, 5, 1, seed=197, affine=True, u_prev=False, bounds=None, du_bound=None, scale=0.2)
+    C = rng.normal(size=(2, 3)); Ly = rng.normal(size=(2, 2)); Wy = Ly @ Ly.T + 0.3 * np.eye(2)
+    Lu = rng.normal(size=(2, 2)); Wu = Lu @ Lu.T + 0.2 * np.eye(2)
+    ry = rng.normal(size=2); ru = 0.3 * rng.normal(size=2)
+    Q, R, qbar = oracle.tracking(C, Wy, Wu, ry, ru)
+    np.testing.assert_allclose(Q, Q.T, atol=1e-15)
+    args = p.instance(0); args.update(Q=Q, R=R, qbar=qbar, P=None)
+    r = oracle.solve(**args, max_iters=60000, tol=1e-24)
+    xs, us = ref.tracking_least_squares(p.A[0], p.B[0], C, Wy, Wu, ry, ru, p.x0[0], e=p.e[0])
+    np.testing.assert_allclose(r.x, xs, atol=1e-8)
+    np.testing.assert_allclose(r.u, us, atol=1e-8)
+    # AFTI-16 (PAPER.md:321-329)
+    Ac = np.array([[-0.0151, -60.5651, 0.0, -32.174], [-0.0001, -1.3411, 0.9929, 0.0], [0.00018, 43.2541, -0.86939, 0.0],
+                   [0.0, 0.0, 1.0, 0.0]])
+    Bc = np.array([[-2.516, -13.136], [-0.1689, -0.2514], [-17.251, -1.5766], [0.0, 0.0]])
+    Cy = np.array([[0.0, 1.0, 0.0, 0.0], [0.0, 0.0, 0.0, 1.0]])
+    N, Ts = 5, 0.05
+    A = np.tile(np.eye(4) + Ts * Ac, (N, 1, 1)); B = np.tile(Ts * Bc, (N, 1, 1))
+    Q, R, qbar = oracle.tracking(Cy, np.diag([100.0, 100.0]), np.zeros((2, 2)), [0.0, 10.0], None)
+    lo = np.array([-np.inf, -0.5, -np.inf, -100.0, -25.0, -25.0]); hi = -lo
+    Wdu = np.diag([0.1, 0.1])
+    r = oracle.solve(A, B, Q, R, lo, hi, np.zeros(4), Wdu=Wdu, qbar=qbar, rho=10.0, max_iters=200000, tol=1e-20)
+    assert r.c_last < 1e-20 and 1000 < r.iters                 # thousands of iterations, as PAPER.md:331 reports
+    xs, us = ref.slsqp_qp(A, B, Q, R, lo, hi, np.zeros(4), Wdu=Wdu, qbar=qbar)
+    assert np.min(np.abs(np.abs(r.x[:, 1]) - 0.5)) < 1e-7      # the output constraint on y_1 is active
+    np.testing.assert_allclose(r.x, xs, atol=5e-5, rtol=1e-5)
+    np.testing.assert_allclose(r.u, us, atol=5e-5, rtol=1e-5)
