@@ -7,13 +7,14 @@
 //     is a "ghost" whose xbar_{k0} = H_{k0-1} h_{k0-1} is recomputed here (its H is resident too), and the
 //     stage after the range is a ghost that only supplies w_{k1}.  The ghosts' iterates (z, theta) /
 //     (z, v, lambda) arrive from the neighbour CTA as tagged words in global memory.
-//   * The ONLY global exchange per iteration is data-flow, not a barrier: every CTA publishes its partial
-//     sum of c (step 4) and its boundary iterates as {value, iteration tag} words
-//     (8-byte single-copy-atomic stores, no fences); a communication warp polls the partials of all
-//     CTAs, sums them in a fixed order (bit-identical in every CTA) and every thread takes the same
-//     accept / restart decision (steps 5-7).  Buffers are double-buffered on the
-//     iteration parity: a CTA cannot run two iterations ahead of a neighbour because it needs that
-//     neighbour's next partial first.
+//   * The ONLY global exchange per iteration is data-flow, not a barrier: every CTA publishes its boundary
+//     iterates as {value, iteration tag} words (8-byte single-copy-atomic stores, no fences) and ADDS its
+//     partial sum of c (step 4), split into three fixed-point limbs, to three L2 words with
+//     relaxed 64-bit atomics; integer sums are exact and order-independent, each word counts its arrivals in
+//     its top bits, and a communication warp per CTA spins until the three words are complete: bit-identical c
+//     in every CTA, so every thread takes the same accept / restart decision (steps 5-7).
+//     Buffers are double-buffered on the iteration parity: a CTA cannot run two iterations ahead of a
+//     neighbour because it needs that neighbour's next contribution first.
 // The launch is cooperative only to guarantee co-residency of the polling CTAs.  Short horizons run as ONE thread-block
 // cluster instead (template flag CL): the same tagged words are pushed into the peers' shared memory (DSMEM) and polled locally.
 #include <algorithm>
@@ -89,6 +90,42 @@ template <> struct Tagged<double> {
     }
 };
 
+// ---- exact, order-independent sum of the CTAs' partials of c through L2 atomics, no fences --------------------------
+// A non-negative double is split into three 47-bit limbs at fixed binary points 2^-7, 2^-54, 2^-101 (it has 53 significant
+// bits, so the split is exact between 2^-101 and 2^40); integer additions are associative, so the 64-bit atomic sums of the
+// limbs over up to 255 CTAs are EXACT and independent of the arrival order: every CTA reads the same integers and rounds
+// them to the same double.  Each limb word carries its own arrival count in its top 8 bits, so a word validates itself
+// (like the tagged words of the halo exchange) and relaxed accesses suffice.  The words are never reset: in a later use of
+// the same parity slot a CTA adds (new limb - its old limb) + one count, so the payload stays the sum of the CURRENT
+// contributions (< 2^56 even while old and new ones are mixed) and the count advances by the grid size per use, modulo 256.
+// A borrow from a transiently negative payload can only make the count look one too SMALL, never complete too early.
+// One relaxed reduction per limb and a spin on three adjacent words replace the all-to-all of tagged partials.
+struct Limbs { unsigned long long l[3]; };
+__device__ __forceinline__ Limbs to_limbs(double s)
+{
+    Limbs r;
+    s = fmin(fmax(s, 0.0), 1.0e12);                            // 2^40 > 1e12: the top limb stays below 2^47
+    const double a = s * 128.0, fa = floor(a);                 // binary point 2^-7
+    const double b = (a - fa) * 140737488355328.0, fb = floor(b);      // 2^47: binary point 2^-54
+    const double c = (b - fb) * 140737488355328.0;             // binary point 2^-101
+    r.l[2] = (unsigned long long)fa; r.l[1] = (unsigned long long)fb; r.l[0] = (unsigned long long)floor(c);
+    return r;
+}
+__device__ __forceinline__ double from_limbs(unsigned long long l0, unsigned long long l1, unsigned long long l2)
+{
+    return (double)l2 * (1.0 / 128.0) + ((double)l1 * 5.551115123125783e-17 /* 2^-54 */ + (double)l0 * 3.944304526105059e-31 /* 2^-101 */);
+}
+__device__ __forceinline__ void red_add_relaxed(unsigned long long *p, unsigned long long v)
+{
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long *p)
+{
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // shared-memory address of the same variable in the CTA of rank `rank` of the cluster
 __device__ __forceinline__ uint32_t map_peer(const void *local, uint32_t rank)
 {
@@ -141,11 +178,8 @@ struct OCfg {
     // exchange buffers per CTA and parity (tagged words): to the left neighbour (z, v, lambda) of the first stage,
     // to the right neighbour (z, theta) of the last stage
     static constexpr int HALO = 5 * LPS;
-    // every partial of c sits in its own 256-byte granule: the polls of all CTAs spread over the L2 slices
-    static constexpr int PSTRIDE = 16;                         // in 16-byte tagged words
-    // replicas of the broadcast c; largest all-to-all grid.  Measured on B200 inside this kernel (C3, N = 1000, 148 CTAs):
-    // all-to-all 3.2 us/iteration, gather + broadcast 4.0 us/iteration, so the two-hop path is kept for grids > 160 only.
-    static constexpr int NREP = 8, A2A_MAX = 160;
+    // L2 path: two parity slots of three limb words for the exact atomic sum of c, 256 bytes apart (see to_limbs)
+    static constexpr int PSTRIDE = 16, NREP = 8;               // sizing of the exchange buffer, in 16-byte words
 };
 
 template <typename T> struct OState { T z, v, th, be, la, d, de; };
@@ -249,6 +283,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     T kap = (T)0;
     int jacc = 0, it_done = 0, restarts = 0;
     bool done = false;
+    unsigned long long xold[2][3] = {{0ull, 0ull, 0ull}, {0ull, 0ull, 0ull}};     // this CTA's limbs still inside the two parity slots
     __syncthreads();
     if (CL) cluster_sync_all();                  // every CTA of the cluster has zeroed its inbound words
 
@@ -411,10 +446,6 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             sum = lane < ncw ? red[lane] : 0.0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            // small grids: every CTA polls every partial (one hop).  Large grids: CTA 0 gathers, sums and publishes c
-            // in NREP replicas, the others poll one replica (two hops, but 148 x 148 polls would take longer).
-            typename TD::W *pp = part + (size_t)par * (G + C::NREP) * C::PSTRIDE;
-            const bool a2a = G <= C::A2A_MAX;
             if (CL) {                                  // push the partial into every CTA of the cluster, poll the own copies
                 if (lane < G) TD::st_cl(map_peer(xPart + par * C::CLMAX + cta, lane), sum, tag);
                 double val = 0.0;
@@ -422,29 +453,24 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 sum = val;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            } else if (a2a || cta == 0) {
-                if (lane == 0) TD::st(pp + (size_t)cta * C::PSTRIDE, sum, tag);
-                double vals[C::MAXJ];
-                bool got[C::MAXJ];
-#pragma unroll
-                for (int u = 0; u < C::MAXJ; ++u) { vals[u] = 0.0; got[u] = lane + 32 * u >= G; }
-                bool all;
-                do {
-                    all = true;
-#pragma unroll
-                    for (int u = 0; u < C::MAXJ; ++u) {
-                        if (!got[u]) { got[u] = TD::ld(pp + (size_t)(lane + 32 * u) * C::PSTRIDE, tag, vals[u]); all = all && got[u]; }
-                    }
-                } while (!all);
-                sum = 0.0;
-#pragma unroll
-                for (int u = 0; u < C::MAXJ; ++u) sum += vals[u];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-                if (!a2a && lane < C::NREP) TD::st(pp + (size_t)(G + lane) * C::PSTRIDE, sum, tag);
             } else {
-                if (lane == 0) TD::st(pp + (size_t)cta * C::PSTRIDE, sum, tag);
-                if (lane == 0) while (!TD::ld(pp + (size_t)(G + cta % C::NREP) * C::PSTRIDE, tag, sum)) {}
+                // exact fixed-point atomic sum (see to_limbs): parity slot, three adjacent words, never reset
+                unsigned long long *acc = reinterpret_cast<unsigned long long *>(part) + (size_t)par * 32;
+                if (lane == 0) {
+                    const Limbs L = to_limbs(sum);
+                    const unsigned expect = (unsigned)((it / 2 + 1) * G) & 255u;              // arrivals in this slot so far, mod 256
+                    const unsigned long long one = 1ull << 56, mask = one - 1;
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {
+                        red_add_relaxed(acc + q, L.l[q] - xold[par][q] + one);
+                        xold[par][q] = L.l[q];
+                    }
+                    unsigned long long v0, v1, v2;
+                    do {
+                        v0 = ld_relaxed(acc); v1 = ld_relaxed(acc + 1); v2 = ld_relaxed(acc + 2);
+                    } while ((unsigned)(v0 >> 56) != expect || (unsigned)(v1 >> 56) != expect || (unsigned)(v2 >> 56) != expect);
+                    sum = from_limbs(v0 & mask, v1 & mask, v2 & mask);
+                }
                 sum = __shfl_sync(0xffffffffu, sum, 0);
             }
             if (lane == 0) red[32 + par] = p.rho * sum;
