@@ -210,10 +210,10 @@ def cstr_closed_loop(torch, pimpc, N=5000, K=1000, steps=6):
     out = {}
     for dt in ("f64", "f32"):
         x = np.array(wl.CSTR["x_init"]); u = np.array([wl.CSTR["u_init"]]); t = 0.0
-        s = pimpc.Solver(4, 2, N, 1, dtype=dt)
+        s = pimpc.Solver(2, 1, N, 1, dtype=dt)
         ms, ca = [], []
         for step in range(steps):
-            pp = wl.pad_problem(wl.cstr_problem(x, u, t, N, iters=K), 4, 2)
+            pp = wl.cstr_problem(x, u, t, N, iters=K)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             s.set_problem(pp)
@@ -230,29 +230,54 @@ def cstr_closed_loop(torch, pimpc, N=5000, K=1000, steps=6):
         out[dt] = {"ms_per_mpc_step_median": statistics.median(ms[1:]), "ms_per_mpc_step_max": max(ms[1:]),
                    "iter_kernel_ms": info["iter_ms"], "cache_kernel_ms": info["setup_ms"], "engine": info["engine"],
                    "grid": info["grid"], "C_A_after_steps": ca[-1]}
-    out["config"] = {"N": N, "iters_per_step": K, "steps_timed": steps - 1, "shape": "(2,1) embedded in (4,2)",
+    out["config"] = {"N": N, "iters_per_step": K, "steps_timed": steps - 1, "shape": "(2,1), the paper's own shape",
                      "paper_gpu_s_per_step": 0.526}
     return out
 
 
-def extras(torch, pimpc, pk):
+def extras(torch, pimpc, pk, only=None):
+    """`only`: comma-separated subset of C1,C2,C3,CSTR,T1,C5 (profiling aid: `--only-extras --extras C5`)."""
+    want = lambda name: only is None or name in only.split(",")
     out = {}
-    out["C1_f64"] = us_per_iteration(torch, pimpc, wl.config1(), "f64", 500)
-    for dt in ("f64", "f32"):
-        out[f"C2_{dt}"] = us_per_iteration(torch, pimpc, wl.config2(), dt, 2000)
+    if want("C1"):
+        out["C1_f64"] = us_per_iteration(torch, pimpc, wl.config1(), "f64", 500)
+    if want("C2"):
+        for dt in ("f64", "f32"):
+            out[f"C2_{dt}"] = us_per_iteration(torch, pimpc, wl.config2(), dt, 2000)
+    if want("C3"):
+        out.update(extras_c3(torch, pimpc))
+    if want("CSTR"):
+        out["CSTR_closed_loop"] = cstr_closed_loop(torch, pimpc)
+    if want("T1"):
+        out["paper_table1_us_per_iter_f64"] = extras_table1(torch, pimpc)
+    if want("C5"):
+        out.update(extras_c5(torch, pimpc, pk))
+    return out
+
+
+def extras_c3(torch, pimpc):
+    out = {}
     sweep = {}
     for N in wl.C3_HORIZONS:
         sweep[str(N)] = us_per_iteration(torch, pimpc, wl.config3(N), "f32", 1000, reps=5)
     out["C3_f32_us_per_iter_vs_N"] = sweep
     out["C3_flatness_t10000_over_t10"] = sweep["10000"]["us_per_iter"] / max(sweep["10"]["us_per_iter"], 1e-9)
-    out["CSTR_closed_loop"] = cstr_closed_loop(torch, pimpc)
+    out["C3_flatness_t10000_over_t100"] = sweep["10000"]["us_per_iter"] / max(sweep["100"]["us_per_iter"], 1e-9)
+    return out
+
+
+def extras_table1(torch, pimpc):
     # the paper's Table I grid (PAPER.md:401-433; its GPU code: 530-620 us per iteration at every size)
     t1 = {}
     for nx, nu in wl.TABLE1_SHAPES:
         for N in wl.TABLE1_HORIZONS:
             r = us_per_iteration(torch, pimpc, wl.paper_random(nx, nu, N), "f64", 200, reps=3)
             t1[f"{nx},{nu},{N}"] = round(r["us_per_iter"], 2)
-    out["paper_table1_us_per_iter_f64"] = t1
+    return t1
+
+
+def extras_c5(torch, pimpc, pk):
+    out = {}
     p5 = wl.config5()
     for dt, esz in (("f32", 4), ("f64", 8)):
         s = pimpc.Solver(p5.nx, p5.nu, p5.N, p5.batch, dtype=dt, rho=p5.rho)
@@ -278,6 +303,7 @@ def main():
     ap.add_argument("--engine", default="auto")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--only-extras", action="store_true", help="run only the C1-C3, C5 legs and print their JSON (profiling aid)")
+    ap.add_argument("--extras", default=None, help="comma-separated subset of the extras: C1,C2,C3,CSTR,T1,C5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -292,7 +318,7 @@ def main():
     pk = peaks()
     if args.only_extras:
         if rank == 0:
-            print(json.dumps({"extras": extras(torch, pimpc, pk)}))
+            print(json.dumps({"extras": extras(torch, pimpc, pk, args.extras)}))
         return 0
 
     lo, hi = replicas.weak_instance_range(BATCH, rank)
@@ -390,15 +416,16 @@ def main():
                 "kernel": "STAGED engine: 5 kernels per iteration (k_hat,k_adj,k_primal,k_dual,k_decide)", "traffic": None}
     else:
         fl = flops_per_stage_iter(prob.nx, prob.nu) * nst * ITERS
-        roof = {"bound": "alu", "achieved": fl / k_ms / 1e9, "peak": onchip["ffma2_tflops"],
-                "unit": "TFLOP/s", "kernel": "k_resident<float,12,4> (one persistent launch per solve)", "traffic": None,
+        roof = {"bound": "alu", "achieved": fl / k_ms / 1e9, "peak": max(onchip["ffma2_tflops"], onchip["ffma_tflops"]),
+                "unit": "TFLOP/s", "kernel": "k_res2<float,12,4> (RESIDENT engine: one persistent launch per solve)", "traffic": None,
                 "peak_nominal": alu_peak_tflops("f32", pk["sm_max_mhz"]), "measured_onchip_peaks": onchip,
                 "algorithmic_GBps_if_streamed": bytes_per_stage_iter(prob.nx, prob.nu, 4) * nst * ITERS / k_ms / 1e6}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["peak_source"] = ("MEASURED_PEAKS.json hbm_gbs" if pk["source"] == "measured" else "fallback hbm_gbs") \
         if roof["bound"] == "hbm" else \
-        "pimpc_measure_peaks(): packed-FFMA2 dependency-chain microbenchmark run on this GPU just before the timed region " \
-        "(the FMA pipe binds: DESIGN.md section 6; shared-memory peak in measured_onchip_peaks)"
+        "pimpc_measure_peaks(): FP32 FMA dependency-chain microbenchmarks (scalar FFMA and packed FFMA2; the larger one) run " \
+        "on this GPU just before the timed region (the FMA pipe binds phases B and C: DESIGN.md section 6; the measured " \
+        "shared-memory peak is in measured_onchip_peaks)"
     roof["kernel_ms_per_launch"] = k_ms
     roof["cache_kernel_ms"] = statistics.mean(setup_ms)
     roof["traffic"] = ncu_traffic(engine, "C4_f32")
@@ -430,7 +457,7 @@ def main():
     for h, _ in pair:
         h.close()
     if world == 1 and not args.no_extras:
-        out["extras"] = extras(torch, pimpc, pk)
+        out["extras"] = extras(torch, pimpc, pk, args.extras)
     print(json.dumps(out))
     return 0
 

@@ -15,6 +15,8 @@
 //     in every CTA, so every thread takes the same accept / restart decision (steps 5-7).
 //     Buffers are double-buffered on the iteration parity: a CTA cannot run two iterations ahead of a
 //     neighbour because it needs that neighbour's next contribution first.
+// The shape is PADDED at compile time (NX x-rows, NU u-rows, multiples of 4); the real nx <= NX, nu <= NU are run-time:
+// pad rows and columns carry zero matrices, zero bounds and zero iterates, run the same instructions and stay exactly 0.
 // The launch is cooperative only to guarantee co-residency of the polling CTAs.  Short horizons run as ONE thread-block
 // cluster instead (template flag CL): the same tagged words are pushed into the peers' shared memory (DSMEM) and polled locally.
 #include <algorithm>
@@ -211,21 +213,24 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     const bool comm = warp == ncw;
     const int ngroups = ncw * (32 / LPS);
     const int g = tid / LPS, li = tid % LPS;
-    const int N = p.N, G = gridDim.x, cta = blockIdx.x;
+    const int N = p.N, G = gridDim.x, cta = blockIdx.x, nx = p.nx, nu = p.nu, nb = p.nb;
+    // padded row / column index -> index in the caller's arrays (-1: pad)
+    auto gidx = [&](int i) -> int { return i < NX ? (i < nx ? i : -1) : (i - NX < nu ? nx + (i - NX) : -1); };
+    const int gi = li < NB ? gidx(li) : -1;
     const int k0 = (int)((long long)cta * N / G), k1 = (int)((long long)(cta + 1) * N / G), L = k1 - k0;
     const bool has_left = k0 > 0, has_right = k1 < N;
     const T rho = (T)p.rho;
     const bool has_e = p.e != nullptr, has_q = p.has_q != 0;
-    const bool rowok = li < NB, isx = li < NX || !rowok;       // pad lanes take the x-row path with zeros
+    const bool rowok = gi >= 0, isx = li < NX || !rowok;       // pad lanes take the x-row path with zeros
     const int i_cur = p.ctl[0].i_cur;
 
     // ---- once per solve: stage matrices -> shared memory, iterates -> registers ----------------------------
     for (int i = tid; i < (L + 2) * SS; i += blockDim.x) sBlk[i] = (T)0;
     for (int i = tid; i < min(iters + 1, C::KAPN); i += blockDim.x) sKap[i] = (T)kappa_tab[i];
-    if (tid < LPS) sQ[tid] = tid < NB ? p.qbar[tid] : (T)0;
+    if (tid < LPS) { const int g0 = tid < NB ? gidx(tid) : -1; sQ[tid] = g0 >= 0 ? p.qbar[g0] : (T)0; }
     if (tid < NUP) {
-        sDlo[tid] = (DU && tid < NU) ? p.dlo[tid] : (T)0;
-        sDhi[tid] = (DU && tid < NU) ? p.dhi[tid] : (T)0;
+        sDlo[tid] = (DU && tid < nu) ? p.dlo[tid] : (T)0;
+        sDhi[tid] = (DU && tid < nu) ? p.dhi[tid] : (T)0;
     }
     if (tid == 0) { red[32] = p.c0; red[33] = p.c0; }
     if (CL) {
@@ -237,17 +242,29 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         if (k < 0 || k >= N) continue;
         T *blk = sBlk + (size_t)v * SS;
         if (v <= L)                                            // H_k: real stages and the left ghost
-            for (int i = tid; i < NB * NB; i += blockDim.x) blk[OHM + (i / NB) * HS + i % NB] = p.H[(size_t)k * NB * NB + i];
+            for (int i = tid; i < NB * NB; i += blockDim.x) {
+                const int gr = gidx(i / NB), gc = gidx(i % NB);
+                blk[OHM + (i / NB) * HS + i % NB] = (gr >= 0 && gc >= 0) ? p.H[(size_t)k * nb * nb + gr * nb + gc] : (T)0;
+            }
         if (v >= 1) {                                          // [A_k B_k], e_k: real stages and the right ghost
-            for (int i = tid; i < NX * NX; i += blockDim.x) blk[OAB + (i / NX) * HS + i % NX] = p.A[(size_t)k * NX * NX + i];
-            for (int i = tid; i < NX * NU; i += blockDim.x) blk[OAB + (i / NU) * HS + NX + i % NU] = p.B[(size_t)k * NX * NU + i];
-            if (has_e && tid < NX) blk[OE + tid] = p.e[(size_t)k * NX + tid];
+            for (int i = tid; i < NX * NB; i += blockDim.x) {
+                const int r = i / NB, c = i % NB, gc = gidx(c);
+                T val = (T)0;
+                if (r < nx && gc >= 0) val = c < NX ? p.A[(size_t)k * nx * nx + r * nx + gc] : p.B[(size_t)k * nx * nu + r * nu + (gc - nx)];
+                blk[OAB + r * HS + c] = val;
+            }
+            if (has_e && tid < nx) blk[OE + tid] = p.e[(size_t)k * nx + tid];
         }
         if (v >= 1 && v <= L)
-            for (int i = tid; i < NU * NU; i += blockDim.x) blk[OMM + (i / NU) * NUP + i % NU] = p.M[(size_t)k * NU * NU + i];
+            for (int i = tid; i < NU * NU; i += blockDim.x) {
+                const int r = i / NU, c = i % NU;
+                blk[OMM + r * NUP + c] = (r < nu && c < nu) ? p.M[(size_t)k * nu * nu + r * nu + c] : (T)0;
+            }
     }
-    if (!has_left && tid < LPS)                                // slot 0 of the first CTA: xbar_0 = (x(t); u(t-1))
-        sBlk[OX + tid] = tid < NX ? p.x0[tid] : (tid < NB ? p.uprev[tid - NX] : (T)0);
+    if (!has_left && tid < LPS) {                              // slot 0 of the first CTA: xbar_0 = (x(t); u(t-1))
+        const int g0 = tid < NB ? gidx(tid) : -1;
+        sBlk[OX + tid] = g0 < 0 ? (T)0 : (tid < NX ? p.x0[g0] : p.uprev[g0 - nx]);
+    }
 
     OState<T> sa[SPG], sb[SPG];
     T lo[SPG], hi[SPG];
@@ -264,16 +281,16 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         const bool ok = (real[s] || ghl[s] || ghr[s]) && rowok;
         const T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(0, ok ? k : 0);
         const bool oku = ok && li >= NX;
-        sa[s].z = ok ? rec[p.oZ() + li] : (T)0;
-        sa[s].v = ok ? rec[p.oV() + li] : (T)0;
-        sa[s].th = ok ? rec[p.oTH() + li] : (T)0;
-        sa[s].be = ok ? rec[p.oBE() + li] : (T)0;
-        sa[s].la = ok ? rec[p.oLA() + li] : (T)0;
-        sa[s].d = (oku && DU) ? rec[p.oD() + (li - NX)] : (T)0;
-        sa[s].de = (oku && DU) ? rec[p.oDE() + (li - NX)] : (T)0;
+        sa[s].z = ok ? rec[p.oZ() + gi] : (T)0;
+        sa[s].v = ok ? rec[p.oV() + gi] : (T)0;
+        sa[s].th = ok ? rec[p.oTH() + gi] : (T)0;
+        sa[s].be = ok ? rec[p.oBE() + gi] : (T)0;
+        sa[s].la = ok ? rec[p.oLA() + gi] : (T)0;
+        sa[s].d = (oku && DU) ? rec[p.oD() + (gi - nx)] : (T)0;
+        sa[s].de = (oku && DU) ? rec[p.oDE() + (gi - nx)] : (T)0;
         sb[s] = sa[s];
-        lo[s] = (real[s] && rowok) ? p.lo[li] : (T)0;
-        hi[s] = (real[s] && rowok) ? p.hi[li] : (T)0;
+        lo[s] = (real[s] && rowok) ? p.lo[gi] : (T)0;
+        hi[s] = (real[s] && rowok) ? p.hi[gi] : (T)0;
     }
     const int hrow = rowok ? li : NB - 1;                      // clamped row indices of pad / u lanes (results unused)
     const int xrow = li < NX ? li : NX - 1;
@@ -534,12 +551,12 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         if (!(real[s] && rowok)) continue;
         const int k = k0 - 1 + s * ngroups + g;
         T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(0, k);
-        rec[p.oZ() + li] = sa[s].z; rec[p.oV() + li] = sa[s].v; rec[p.oTH() + li] = sa[s].th;
-        rec[p.oBE() + li] = sa[s].be; rec[p.oLA() + li] = sa[s].la;
-        p.X[(size_t)k * NB + li] = blkp[s][OX + li];
+        rec[p.oZ() + gi] = sa[s].z; rec[p.oV() + gi] = sa[s].v; rec[p.oTH() + gi] = sa[s].th;
+        rec[p.oBE() + gi] = sa[s].be; rec[p.oLA() + gi] = sa[s].la;
+        p.X[(size_t)k * nb + gi] = blkp[s][OX + li];
         if (li >= NX) {
-            p.DU[(size_t)k * NU + (li - NX)] = blkp[s][ODU + li - NX];
-            if (DU) { rec[p.oD() + (li - NX)] = sa[s].d; rec[p.oDE() + (li - NX)] = sa[s].de; }
+            p.DU[(size_t)k * nu + (gi - nx)] = blkp[s][ODU + li - NX];
+            if (DU) { rec[p.oD() + (gi - nx)] = sa[s].d; rec[p.oDE() + (gi - nx)] = sa[s].de; }
         }
     }
     if (cta == 0 && tid == 0) {
@@ -656,19 +673,21 @@ int run_coop_t(pimpc_s *h, int iters, double tol)
     return n < 0 ? n : n + launches;
 }
 
-bool coop_shape(const pimpc_s *h) { return (h->nx == 12 && h->nu == 4) || (h->nx == 4 && h->nu == 2); }
+// padded shapes with an instantiation: (4, 4) and (12, 4); any nx <= 12, nu <= 4 runs inside the smallest that holds it
+bool coop_shape(const pimpc_s *h) { return h->nx <= 12 && h->nu <= 4; }
+bool coop_small(const pimpc_s *h) { return h->nx <= 4; }
 
 } // namespace
 
 bool coop_supported(const pimpc_s *h, std::string *why)
 {
     if (h->batch != 1) { if (why) *why = "COOP engine is for batch = 1"; return false; }
-    if (!coop_shape(h)) { if (why) *why = "no COOP instantiation for this (nx, nu)"; return false; }
+    if (!coop_shape(h)) { if (why) *why = "no COOP instantiation holds this (nx, nu) (nx <= 12, nu <= 4)"; return false; }
     if (h->bnd_per_instance || h->cost_per_instance) { /* batch = 1: strides are irrelevant */ }
     CoopPlan pl;
     const bool d = h->dtype == PIMPC_F64;
-    if (h->nx == 12) return d ? plan_coop<double, 12, 4>(h, &pl, why) : plan_coop<float, 12, 4>(h, &pl, why);
-    return d ? plan_coop<double, 4, 2>(h, &pl, why) : plan_coop<float, 4, 2>(h, &pl, why);
+    if (!coop_small(h)) return d ? plan_coop<double, 12, 4>(h, &pl, why) : plan_coop<float, 12, 4>(h, &pl, why);
+    return d ? plan_coop<double, 4, 4>(h, &pl, why) : plan_coop<float, 4, 4>(h, &pl, why);
 }
 
 int run_coop(pimpc_s *h, int iters, double tol)
@@ -676,6 +695,6 @@ int run_coop(pimpc_s *h, int iters, double tol)
     std::string why;
     if (!coop_supported(h, &why)) { h->errmsg = "COOP engine not applicable: " + why; return PIMPC_EINVAL; }
     const bool d = h->dtype == PIMPC_F64;
-    if (h->nx == 12) return d ? run_coop_t<double, 12, 4>(h, iters, tol) : run_coop_t<float, 12, 4>(h, iters, tol);
-    return d ? run_coop_t<double, 4, 2>(h, iters, tol) : run_coop_t<float, 4, 2>(h, iters, tol);
+    if (!coop_small(h)) return d ? run_coop_t<double, 12, 4>(h, iters, tol) : run_coop_t<float, 12, 4>(h, iters, tol);
+    return d ? run_coop_t<double, 4, 4>(h, iters, tol) : run_coop_t<float, 4, 4>(h, iters, tol);
 }

@@ -154,7 +154,9 @@ struct Cursor {
     __device__ void next(const Seg *seg) { if (++o >= seg[sg].nsteps) { o = 0; ++sg; } }
 };
 
-template <typename T, int NX, int NU>
+// EXT: per-stage boxes / linear terms or a general convex set are present (pimpc_set_stage_terms, pimpc_set_tracking with
+// per-stage references, pimpc_set_constraint); the plain variant carries none of their address arithmetic or barriers.
+template <typename T, int NX, int NU, bool EXT>
 __global__ void __launch_bounds__(SCfg<T, NX, NU>::NT)
 k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ partial, const int iters, const int nslot, const int span)
 {
@@ -176,7 +178,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
     const long long s0 = cta * S_tot / G, s1 = (cta + 1) * S_tot / G;
     const int b_first = (int)(s0 / N1), n_local = (int)((s1 - 1) / N1) - b_first + 1;
     const T rho = (T)p.rho;
-    const bool has_du = p.has_du != 0, has_q = p.has_q != 0, gset = p.set_kind != PIMPC_SET_NONE;
+    const bool has_du = p.has_du != 0, has_q = p.has_q != 0, gset = EXT && p.set_kind != PIMPC_SET_NONE;
     const int ci = tid % IP, prt = tid / IP;              // column index / row-range part of the column products
     const int di = tid - 4 * NX;                           // component of the dual update (threads >= 4 NX)
 
@@ -337,7 +339,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         if (i >= NX) g += wv[i];                                    // the [0 I] rows of Abar_{j+1}
                         h += rho * g;
                     }
-                    if (has_q) h += p.qbar_at(b, j, i);
+                    if (has_q) h += EXT ? p.qbar_at(b, j, i) : p.qbar[(size_t)b * p.qbar_stride + i];
                     hv[i] = h; hv[i + NB] = h;
                 }
                 if (tid >= IP && tid < IP + NU && do_next) {
@@ -409,50 +411,92 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         avc[pn * IP + r] = s1_ + hs[3 * NB + r];                   // a = Bbar du + betahat
                     }
                 }
-                const bool dthread = di >= 0 && di < NB;
-                if (dthread && do_next && di >= NX) {
-                    bc[pn * IP + di] = xv[di] - hs[4 * NB + di];
-                    avc[pn * IP + di] = duc[pn * IP + di - NX] + hs[3 * NB + di];
-                }
-                // argument of Proj of stage j (Thm 1, proof form, R1); with a general set (pimpc_set_constraint) the whole
-                // vector is staged in shared memory first (xp is free after phase E) -- a CTA-uniform extra barrier
-                T zarg = (T)0;
-                if (dthread && do_dual) {
-                    const int i = di;
-                    const T av = avc[pj * IP + i], bv = bc[pj * IP + i];
-                    zarg = ((T)2 * (xv[i] + hj[2 * NB + i] + bv) + (av - bv)) * (T)(1.0 / 3.0);
-                    if (gset) xp[i] = zarg;
-                }
-                if (gset && do_dual) __syncthreads();
-                if (dthread) {
-                    const int i = di;
-                    if (do_dual) {
-                        const T zh = hj[i], vh = hj[NB + i], thh = hj[2 * NB + i], beh = hj[3 * NB + i], lah = hj[4 * NB + i];
-                        const T av = avc[pj * IP + i], bv = bc[pj * IP + i], x = xv[i];
-                        const T gam = av - bv;
-                        T zn;
-                        if (gset && i >= p.set_i0 && i < p.set_i0 + p.set_len) zn = proj_set_component(p, xp + p.set_i0, i - p.set_i0);
-                        else zn = clips(zarg, p.lo_at(b, j, i), p.hi_at(b, j, i));
-                        const T vn = (T)0.5 * (zn + gam);
-                        const T thn = thh + x - zn, ben = av - vn, lan = zn - bv - vn;
-                        const T d0 = thn - thh, d1 = ben - beh, d2 = lan - lah, d3 = zn - zh, d4 = vn - vh;
-                        const T d5 = (zn - vn) - (zh - vh);
-                        T a = d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
-                        T *nw = p.S + (size_t)L.i_new * p.buf_stride + p.st(b, j);
-                        nw[i] = zn; nw[NB + i] = vn; nw[2 * NB + i] = thn; nw[3 * NB + i] = ben; nw[4 * NB + i] = lan;
-                        if (has_du && i >= NX) {                                   // Delta-u box copy (reading R12)
-                            const int q = i - NX;
-                            const T duq = duc[pj * IP + q], dh = hj[5 * NB + q], deh = hj[5 * NB + NU + q];
-                            const T dn = clips(duq + deh, p.dlo[(size_t)b * p.dbnd_stride + q], p.dhi[(size_t)b * p.dbnd_stride + q]);
-                            const T den = deh + duq - dn;
-                            const T e0 = den - deh, e1 = dn - dh;
-                            a += e0 * e0 + e1 * e1;
-                            nw[5 * NB + q] = dn; nw[5 * NB + NU + q] = den;
+                if constexpr (!EXT) {
+                    if (di >= 0 && di < NB) {
+                        const int i = di;
+                        if (do_next && i >= NX) {
+                            bc[pn * IP + i] = xv[i] - hs[4 * NB + i];
+                            avc[pn * IP + i] = duc[pn * IP + i - NX] + hs[3 * NB + i];
                         }
-                        acc += (double)a;
-                        if (write_x) {
-                            p.X[((size_t)b * N + j) * NB + i] = x;
-                            if (i >= NX) p.DU[((size_t)b * N + j) * NU + (i - NX)] = duc[pj * IP + i - NX];
+                        if (do_dual) {
+                            const T zh = hj[i], vh = hj[NB + i], thh = hj[2 * NB + i], beh = hj[3 * NB + i], lah = hj[4 * NB + i];
+                            const T av = avc[pj * IP + i], bv = bc[pj * IP + i], x = xv[i];
+                            const T lo = p.lo[(size_t)b * p.bnd_stride + i], hi = p.hi[(size_t)b * p.bnd_stride + i];
+                            const T gam = av - bv;
+                            const T zn = clips(((T)2 * (x + thh + bv) + gam) * (T)(1.0 / 3.0), lo, hi);   // Thm 1 (proof form, R1)
+                            const T vn = (T)0.5 * (zn + gam);
+                            const T thn = thh + x - zn, ben = av - vn, lan = zn - bv - vn;
+                            const T d0 = thn - thh, d1 = ben - beh, d2 = lan - lah, d3 = zn - zh, d4 = vn - vh;
+                            const T d5 = (zn - vn) - (zh - vh);
+                            T a = d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
+                            T *nw = p.S + (size_t)L.i_new * p.buf_stride + p.st(b, j);
+                            nw[i] = zn; nw[NB + i] = vn; nw[2 * NB + i] = thn; nw[3 * NB + i] = ben; nw[4 * NB + i] = lan;
+                            if (has_du && i >= NX) {                                   // Delta-u box copy (reading R12)
+                                const int q = i - NX;
+                                const T duq = duc[pj * IP + q], dh = hj[5 * NB + q], deh = hj[5 * NB + NU + q];
+                                const T dn = clips(duq + deh, p.dlo[(size_t)b * p.dbnd_stride + q], p.dhi[(size_t)b * p.dbnd_stride + q]);
+                                const T den = deh + duq - dn;
+                                const T e0 = den - deh, e1 = dn - dh;
+                                a += e0 * e0 + e1 * e1;
+                                nw[5 * NB + q] = dn; nw[5 * NB + NU + q] = den;
+                            }
+                            acc += (double)a;
+                            if (write_x) {
+                                p.X[((size_t)b * N + j) * NB + i] = x;
+                                if (i >= NX) p.DU[((size_t)b * N + j) * NU + (i - NX)] = duc[pj * IP + i - NX];
+                            }
+                        }
+                    }
+                } else {
+                    const bool dthread = di >= 0 && di < NB;
+                    if (dthread && do_next && di >= NX) {
+                        bc[pn * IP + di] = xv[di] - hs[4 * NB + di];
+                        avc[pn * IP + di] = duc[pn * IP + di - NX] + hs[3 * NB + di];
+                    }
+                    // argument of Proj of stage j (Thm 1, proof form, R1); with a general set (pimpc_set_constraint) the whole
+                    // vector is staged in shared memory first (xp is free after phase E) -- a CTA-uniform extra barrier
+                    if constexpr (EXT) {
+                        if (gset && do_dual) {
+                            if (dthread) {
+                                const int i = di;
+                                const T av = avc[pj * IP + i], bv = bc[pj * IP + i];
+                                xp[i] = ((T)2 * (xv[i] + hj[2 * NB + i] + bv) + (av - bv)) * (T)(1.0 / 3.0);
+                            }
+                            __syncthreads();
+                        }
+                    }
+                    if (dthread) {
+                        const int i = di;
+                        if (do_dual) {
+                            const T zh = hj[i], vh = hj[NB + i], thh = hj[2 * NB + i], beh = hj[3 * NB + i], lah = hj[4 * NB + i];
+                            const T av = avc[pj * IP + i], bv = bc[pj * IP + i], x = xv[i];
+                            const T gam = av - bv;
+                            const T zarg = ((T)2 * (x + thh + bv) + gam) * (T)(1.0 / 3.0);
+                            T zn;
+                            if (EXT && gset && i >= p.set_i0 && i < p.set_i0 + p.set_len) zn = proj_set_component(p, xp + p.set_i0, i - p.set_i0);
+                            else if (EXT) zn = clips(zarg, p.lo_at(b, j, i), p.hi_at(b, j, i));
+                            else zn = clips(zarg, p.lo[(size_t)b * p.bnd_stride + i], p.hi[(size_t)b * p.bnd_stride + i]);
+                            const T vn = (T)0.5 * (zn + gam);
+                            const T thn = thh + x - zn, ben = av - vn, lan = zn - bv - vn;
+                            const T d0 = thn - thh, d1 = ben - beh, d2 = lan - lah, d3 = zn - zh, d4 = vn - vh;
+                            const T d5 = (zn - vn) - (zh - vh);
+                            T a = d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
+                            T *nw = p.S + (size_t)L.i_new * p.buf_stride + p.st(b, j);
+                            nw[i] = zn; nw[NB + i] = vn; nw[2 * NB + i] = thn; nw[3 * NB + i] = ben; nw[4 * NB + i] = lan;
+                            if (has_du && i >= NX) {                                   // Delta-u box copy (reading R12)
+                                const int q = i - NX;
+                                const T duq = duc[pj * IP + q], dh = hj[5 * NB + q], deh = hj[5 * NB + NU + q];
+                                const T dn = clips(duq + deh, p.dlo[(size_t)b * p.dbnd_stride + q], p.dhi[(size_t)b * p.dbnd_stride + q]);
+                                const T den = deh + duq - dn;
+                                const T e0 = den - deh, e1 = dn - dh;
+                                a += e0 * e0 + e1 * e1;
+                                nw[5 * NB + q] = dn; nw[5 * NB + NU + q] = den;
+                            }
+                            acc += (double)a;
+                            if (write_x) {
+                                p.X[((size_t)b * N + j) * NB + i] = x;
+                                if (i >= NX) p.DU[((size_t)b * N + j) * NU + (i - NX)] = duc[pj * IP + i - NX];
+                            }
                         }
                     }
                 }
@@ -530,11 +574,11 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
 
 struct StreamPlan { int grid, nslot; size_t smem; };
 
-template <typename T, int NX, int NU>
+template <typename T, int NX, int NU, bool EXT>
 int plan_stream(pimpc_s *h, StreamPlan *pl)
 {
     using C = SCfg<T, NX, NU>;
-    auto kern = k_stream<T, NX, NU>;
+    auto kern = k_stream<T, NX, NU, EXT>;
     const size_t fixed = ((sizeof(StreamSmem) + 127) / 128) * 128 + (size_t)C::V_END * sizeof(T);
     const size_t slot = (size_t)C::SLOT * sizeof(T);
     // CTAs per SM: enough bytes in flight per SM to cover the HBM latency (>= 2 slots per CTA), several
@@ -569,12 +613,12 @@ int plan_stream(pimpc_s *h, StreamPlan *pl)
     return PIMPC_OK;
 }
 
-template <typename T, int NX, int NU>
-int run_stream_t(pimpc_s *h, int iters, double tol)
+template <typename T, int NX, int NU, bool EXT>
+int run_stream_e(pimpc_s *h, int iters, double tol)
 {
     using C = SCfg<T, NX, NU>;
     StreamPlan pl;
-    int rc = plan_stream<T, NX, NU>(h, &pl);
+    int rc = plan_stream<T, NX, NU, EXT>(h, &pl);
     if (rc) return rc;
     int launches = 0;
     const size_t nblob = (size_t)h->batch * (h->N + 1);
@@ -597,9 +641,15 @@ int run_stream_t(pimpc_s *h, int iters, double tol)
     double *partial = h->spartial;
     int nslot = pl.nslot;
     void *args[] = {(void *)&p, (void *)&blob, (void *)&partial, (void *)&iters, (void *)&nslot, (void *)&span};
-    PIMPC_CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)k_stream<T, NX, NU>, dim3(pl.grid), dim3(C::NT), args, pl.smem, h->stream));
+    PIMPC_CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)k_stream<T, NX, NU, EXT>, dim3(pl.grid), dim3(C::NT), args, pl.smem, h->stream));
     h->info.grid = pl.grid; h->info.block = C::NT; h->info.smem_bytes = pl.smem;
     return launches + 1;
+}
+
+template <typename T, int NX, int NU>
+int run_stream_t(pimpc_s *h, int iters, double tol)
+{
+    return has_stage_terms(h) ? run_stream_e<T, NX, NU, true>(h, iters, tol) : run_stream_e<T, NX, NU, false>(h, iters, tol);
 }
 
 // (nx, nu) with a STREAM instantiation: the three BASELINE.json shapes and the paper's Table I shapes

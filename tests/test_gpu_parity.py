@@ -232,19 +232,22 @@ def test_coop_engine_unbounded_plain_admm_early_stop_warm_start(oracle, pimpc, g
 
 
 # ---- NEXT row f1: receding-horizon stepping with shift warm start ----------------
-@pytest.mark.parametrize("engine", ["auto", "coop", "stream", "staged"])
-def test_closed_loop_cstr_shift_warm_start(oracle, pimpc, engine):
+@pytest.mark.parametrize("engine,native", [("auto", True), ("coop", True), ("staged", True), ("resident", True),
+                                           ("stream", False), ("auto", False), ("coop", False)])
+def test_closed_loop_cstr_shift_warm_start(oracle, pimpc, engine, native):
     """Four MPC steps of the online-linearised CSTR: per step new stage data (set_stages + a0), pimpc_shift(1) of the
-    previous iterates, K iterations; the plant advances with the oracle's u_0.  The CUDA path runs the (2, 1)
-    problem embedded in the (4, 2) shape (workloads.pad_problem), the oracle the original one."""
+    previous iterates, K iterations; the plant advances with the oracle's u_0.  native: the CUDA path runs the paper's
+    own (n, m) = (2, 1) shape (PAPER.md:397-399; the fused engines hold it inside their padded (4, 4) instantiation);
+    else the problem is embedded in the (4, 2) shape by workloads.pad_problem (STREAM has no smaller instantiation)."""
     N, K, T = 60, 120, 4
     x = np.array(wl.CSTR["x_init"]); u = np.array([wl.CSTR["u_init"]]); t = 0.0
-    s = pimpc.Solver(4, 2, N, 1, dtype="f64", engine=engine, history=K)
-    real = [0, 1, 4]
+    s = pimpc.Solver(2, 1, N, 1, dtype="f64", engine=engine, history=K) if native else \
+        pimpc.Solver(4, 2, N, 1, dtype="f64", engine=engine, history=K)
+    real = [0, 1, 2] if native else [0, 1, 4]
     warm = None
     for step in range(T):
         p = wl.cstr_problem(x, u, t, N, iters=K)
-        s.set_problem(wl.pad_problem(p, 4, 2))
+        s.set_problem(p if native else wl.pad_problem(p, 4, 2))
         if step:
             s.shift(1)
         s.solve(K)
@@ -255,12 +258,15 @@ def test_closed_loop_cstr_shift_warm_start(oracle, pimpc, engine):
         for name in ("Z", "V", "TH", "BE", "LA", "X"):
             g = s.get_state(name)[0]
             assert parity.relerr(g[:, real], getattr(o, name)) <= 1e-9, (step, name)
-            assert float(np.max(np.abs(np.delete(g, real, axis=1)))) == 0.0          # the embedding stays exactly zero
+            if not native:
+                assert float(np.max(np.abs(np.delete(g, real, axis=1)))) == 0.0      # the embedding stays exactly zero
         xg, ug, dug, res = s.get()
         assert parity.relerr(ug[0, :, :1], o.u) <= 1e-9 and parity.relerr(dug[0, :, :1], o.DU) <= 1e-9
         warm = dict(Z=o.Z, V=o.V, TH=o.TH, BE=o.BE, LA=o.LA)
         u = o.u[0].copy()
         x = wl.cstr_plant_step(x, u, t); t += wl.CSTR["Ts"]
+    if native and engine != "staged":
+        assert s.get_info()["engine"] != pimpc.ENGINE_STAGED      # a fused engine runs the native shape
     assert x[0] < wl.CSTR["x_init"][0]                    # the loop moves C_A towards the reference
 
 

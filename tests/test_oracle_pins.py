@@ -458,3 +458,38 @@ def test_tracking_cost_matches_least_squares_and_afti16_output_box(oracle):
     assert np.min(np.abs(np.abs(r.x[:, 1]) - 0.5)) < 1e-7      # the output constraint on y_1 is active
     np.testing.assert_allclose(r.x, xs, atol=5e-5, rtol=1e-5)
     np.testing.assert_allclose(r.u, us, atol=5e-5, rtol=1e-5)
+
+
+# ----------------------------------------------------------------------------------------------
+# Riccati-ADMM as a second, independent oracle for converged solutions
+# ----------------------------------------------------------------------------------------------
+def test_riccati_admm_primal_step_is_the_lqr_minimiser():
+    """Eq. (6a) by the backward Riccati recursion == one dense KKT solve of the same unconstrained problem."""
+    from oracle import riccati_admm as ra
+    p = wl.random_ltv(3, 2, 6, 1, seed=79, affine=True, u_prev=False, full_cost=True, qbar=True)
+    a = p.instance(0)
+    N, nx = p.N, p.nx
+    Qs = np.stack([a["Q"]] * (N - 1) + [a["P"]])
+    x, u = ra.lqr_step(a["A"], a["B"], a["e"], Qs, np.tile(a["qbar"][:nx], (N, 1)), a["R"], np.tile(a["qbar"][nx:], (N, 1)), a["x0"])
+    U, X = ref.dense_kkt(a["A"], a["B"], a["Q"], a["R"], a["x0"], e=a["e"], P=a["P"], qbar=a["qbar"])
+    np.testing.assert_allclose(u, U, atol=1e-10)
+    np.testing.assert_allclose(x, X, atol=1e-10)
+
+
+def test_two_independent_admm_oracles_agree_at_convergence(oracle):
+    """piMPC (Alg. 1) and Riccati-ADMM (Eq. 5-6) are different splittings of the same QP (1): their converged (x, u)
+    must coincide (and equal the brute-force active-set solution on the tiny case), with x- and u-bounds active."""
+    from oracle import riccati_admm as ra
+    cases = [wl.p_tiny(False), wl.config1(),
+             wl.random_ltv(3, 2, 7, 1, seed=80, affine=True, u_prev=False, qbar=True, bounds=0.7, du_bound=None, scale=0.2)]
+    for p in cases:
+        a = p.instance(0)
+        r = oracle.solve(**a, max_iters=400000, tol=1e-24)
+        assert r.c_last < 1e-24, p.name
+        s = ra.solve(a["A"], a["B"], a["Q"], a["R"], a["lo"], a["hi"], a["x0"], e=a["e"], P=a["P"], qbar=a["qbar"],
+                     rho=1.0, tol=1e-11)
+        assert s["r_prim"] < 1e-11 and s["r_dual"] < 1e-11, (p.name, s["iters"])
+        z = np.hstack([r.x, r.u])
+        assert np.sum(np.isclose(z, a["lo"], atol=1e-8) | np.isclose(z, a["hi"], atol=1e-8)) >= 1, p.name   # a bound is active
+        np.testing.assert_allclose(r.u, s["u"], atol=5e-8, err_msg=p.name)
+        np.testing.assert_allclose(r.x, s["x"], atol=5e-8, err_msg=p.name)
