@@ -427,7 +427,7 @@ int launch_resident(pimpc_s *h, int iters, double tol, int nwarps)
 } // namespace
 
 // The one-row-per-lane kernel above serves fp32 (12, 4) horizons beyond the 13 warps of the two-rows-per-lane kernel
-// (53 <= N <= 64) and opts.tune.rows_per_lane = 1; every other RESIDENT solve runs k_res2 (k_resident2.cu).
+// (61 <= N <= 64: 15 stage warps + the reducer) and opts.tune.rows_per_lane = 1; every other RESIDENT solve runs k_res2 (k_resident2.cu).
 static bool one_row_shape(const pimpc_s *h) { return h->dtype == PIMPC_F32 && h->nx == 12 && h->nu == 4 && h->N <= 64; }
 
 bool resident_supported(const pimpc_s *h, std::string *why)

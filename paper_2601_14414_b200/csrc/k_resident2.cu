@@ -19,10 +19,19 @@
 // element-wise step of Alg. 1 works on both rows at once with packed fp32 instructions (add/mul/fma.f32x2 on sm_100a).
 // Per iteration only five 16-element vectors per stage go through shared memory (w, t, rr out; xbar, Delta u back),
 // read with 16-byte broadcast loads; the slot stride makes those loads and the 8-byte own-row stores conflict-free.
-// Three CTA barriers per iteration.  c (step 4) is reduced in a fixed order: stage sums in T (xor butterfly over the
-// group), warp sums and the sum over warps in double; every thread takes the same accept / restart decision (steps
-// 5-7) from bit-identical numbers.
+// c (step 4) is reduced in a fixed order: stage sums in T (xor butterfly over the group), warp sums and the sum over
+// warps in double; every thread takes the same accept / restart decision (steps 5-7) from bit-identical numbers.
+//
+// The decision is SPECULATED (round 2): steps 5-7 gate the hats of the next iteration, and the
+// reduce -> decide chain was 30 % of an iteration with nothing to overlap it.  Almost every step is accepted, so the
+// kernel forms the next hats with the momentum of an accepted step right after step 4 (own registers only), lets the
+// reduction of c ride along with phases A and B of the next iteration (independent instructions of the same warps) and
+// resolves the decision before phase C, the first point that overwrites an iterate.  A restart repeats A and B with
+// kappa = 0 (hat = new iterate needs `cur` only); a stop returns the iterate phase C has not touched.  Results are the
+// ones of the unspeculated order, bit for bit.  Two CTA barriers per iteration (xbar / Delta u slots alternate by the
+// parity of the iteration, so the stopped iteration's primal step survives the speculated phase B).
 #include <algorithm>
+#include <cstdio>
 
 #include "pimpc_internal.h"
 
@@ -37,10 +46,17 @@ template <> struct Pr<double> { typedef double2 t; };
 
 __device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
+#ifdef R2_SCALAR
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return make_float2(__fmaf_rn(a.x, b.x, c.x), __fmaf_rn(a.y, b.y, c.y)); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return make_float2(__fsub_rn(a.x, b.x), __fsub_rn(a.y, b.y)); }
+#else
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }   // a - b, one rounding
+#endif
 __device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 mul2(double2 a, double2 b) { return make_double2(a.x * b.x, a.y * b.y); }
 __device__ __forceinline__ double2 fma2(double2 a, double2 b, double2 c) { return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
@@ -73,16 +89,16 @@ struct R2Cfg {
     static constexpr int ROWP = 2 * LPS;                      // padded vector length of a stage
     static constexpr int WPE = sizeof(T) / 4;
     static constexpr int KAPN = 1024;                         // kappa table entries cached in smem
-    static constexpr int MAXW = 16;                           // warps per CTA (second reduction level reads 16 partials)
     // One block per stage slot s = k + 1 (slot 0 holds xbar_0, slot NS + 1 a zero w):
     //   W  w_k = zhat - vhat - ebar + lambdahat     T  t_k = qbar + rho (zhat - thetahat)
     //   RR (vhat - betahat) with (dhat - deltahat) added on the u rows      X  xbar_{k+1}      DU Delta u_k
     //   E  e_k per row (read only when present)
     // and once per CTA (the same for every stage): per-row constants B = qbar, du_lo, du_hi, lo, hi
-    //   G  the lane's two rows of G_k, [2][NXP / 4][LPS][4] (a warp's 16-byte loads are contiguous per group, conflict-free):
+    //   G  the lane's two rows of G_k, [2][NXP / 2][LPS][2] (8-byte pieces, lane-major: see ld4p on load widths):
     //      written by the prologue; read every iteration when the rows do not fit in registers (GS: more than 12 warps cap
     //      a thread at 128 registers), else copied to registers once
-    static constexpr int OW = 0, OT = ROWP, ORR = 2 * ROWP, OX = 3 * ROWP, ODU = 4 * ROWP, OE = ODU + NUP, OG = OE + ROWP,
+    // X and DU exist twice (parity of the iteration, see "speculated" above): OX + par * ROWP, ODU + par * NUP
+    static constexpr int OW = 0, OT = ROWP, ORR = 2 * ROWP, OX = 3 * ROWP, ODU = 5 * ROWP, OE = ODU + 2 * NUP, OG = OE + ROWP,
                          SS0 = OG + NXP * ROWP;
     // slot stride == 64 / SPW words (mod 32): shared memory serves 8- and 16-byte accesses one half-warp at a time, and
     // the SPW / 2 groups of a half-warp then hit disjoint banks with their own-row accesses and their broadcast chunks
@@ -92,14 +108,22 @@ struct R2Cfg {
     static constexpr int SSW = SSW0 + ((TGT - SSW0 % 32) + 32) % 32;
     static constexpr int SS = SSW / WPE;
     static_assert(NXP % 4 == 0 && NUP % 4 == 0 && LPS >= 4 && LPS <= 32 && ROWP >= NBP && (SS * sizeof(T)) % 16 == 0 && SSW % WPE == 0, "bad row blocking");
-    static size_t smem_bytes(int nwarps)
+    static size_t smem_bytes(int nmain)                       // nmain = warps that own stages (the CTA has one more: the reducer)
     {
-        const size_t NS = (size_t)nwarps * SPW;
-        return ((NS + 2) * SS + KAPN + 10 * ROWP) * sizeof(T) + 40 * sizeof(double);
+        const size_t NS = (size_t)nmain * SPW;
+        return ((NS + 2) * SS + KAPN + 10 * ROWP + 2 * (size_t)nmain * 32) * sizeof(T) + 8 * sizeof(double);
     }
 };
 
 template <typename P> struct R2State { P z, v, th, be, la, d, de; };
+
+// Phase clock profile of CTA 0 (a -DR2_PROF build for profiles/, never shipped): cycles per phase, warps 0 and last.
+#ifdef R2_PROF
+__device__ long long g_r2prof[1024 * 16 * 8];
+#define R2P(i) do { if (blockIdx.x == 0 && lane == 0 && pit < 1024) g_r2prof[(pit * 16 + warp) * 8 + (i)] = clock64(); } while (0)
+#else
+#define R2P(i) do { } while (0)
+#endif
 
 // GS: the rows of G_k live in shared memory instead of registers (CTAs of 13..16 warps: 4 warps share a sub-partition's
 // 16 K registers, 128 per thread; up to 12 warps get 168).
@@ -113,14 +137,15 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     constexpr int OW = C::OW, OT = C::OT, ORR = C::ORR, OX = C::OX, ODU = C::ODU, OE = C::OE, OG = C::OG, ROWP = C::ROWP;
     constexpr int NG = GS ? 1 : NXP;                          // register copy of G only when it is not in shared memory
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
-    const int NS = nwarps * SPW, N = p.N, nx = p.nx, nu = p.nu, nb = p.nb;
-    double *red = reinterpret_cast<double *>(smem_raw);       // [16] warp partials of c (zero beyond nwarps), [32..33] c of the last two iterations
-    int *sCnt = reinterpret_cast<int *>(red + 34);            // [0] restarts
-    T *sKap = reinterpret_cast<T *>(red + 40);                // [KAPN]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nmain = (blockDim.x >> 5) - 1;                  // warps 0..nmain-1 own stages, warp nmain is the reducer
+    const int NS = nmain * SPW, N = p.N, nx = p.nx, nu = p.nu, nb = p.nb;
+    int *sDec = reinterpret_cast<int *>(smem_raw);            // [0] decision of the reducer: 0 accept, 1 restart, 2 stop
+    T *sKap = reinterpret_cast<T *>(smem_raw + 8 * sizeof(double));   // [KAPN]
     T *sBnd = sKap + C::KAPN;                                 // [5][ROWP] qbar, du_lo, du_hi, lo, hi by padded row, then
                                                               // [5][ROWP] zeros: the constants of the pad stages (k >= N)
-    T *sBlk = sBnd + 10 * ROWP;                               // [NS + 2][SS]
+    T *sAcc = sBnd + 10 * ROWP;                               // [2][nmain * 32] per-lane partial sums of c by parity of the iteration
+    T *sBlk = sAcc + 2 * nmain * 32;                          // [NS + 2][SS]
 
     const int li = lane % LPS, k = warp * SPW + lane / LPS;
     const bool stage_ok = k < N;
@@ -138,11 +163,76 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 
     for (int i = tid; i < (NS + 2) * SS; i += blockDim.x) sBlk[i] = (T)0;      // pads must stay finite zeros
     for (int i = tid; i < min(iters + 1, C::KAPN); i += blockDim.x) sKap[i] = (T)kappa_tab[i];
-    if (tid < 16) red[tid] = 0.0;
     for (int i = tid; i < 5 * ROWP; i += blockDim.x) sBnd[5 * ROWP + i] = (T)0;
     __syncthreads();
 
+#ifdef R2_PROF
+    int pit = 0;
+#endif
     for (int b = blockIdx.x; b < p.batch; b += gridDim.x) {
+        if (warp == nmain) {
+            // ---- the reducer warp: step 4's sum and steps 5-7 for the whole CTA.  It follows the barrier
+            // sequence of the stage warps: per iteration bar1 (phase A published | partial sums of the previous iteration
+            // complete), bar2 (phase B done | decision published), two more after a restart.
+            double c_last = p.c0, c_prev = p.c0, thr = p.eta * p.c0;   // thr = eta c^{i}: ready before c^{i+1} arrives
+            int jacc = 0, nrest = 0, n_it = 0;
+            bool done = false;
+            auto decide = [&](const int it) -> int {
+                // fixed order: this lane's column over the stage warps (all loads in flight at once, zeros beyond nmain, a
+                // balanced tree), then the butterfly over the lanes -- in T: for fp32 handles an fp32 tree of <= 512 partials
+                // (relative error <= 9 * 2^-24, far below the error the partials already carry) keeps the chain at ~230
+                // cycles (a double chain with its conversions took ~700: the stage warps waited for it at barrier 2)
+                const T *a = sAcc + (it & 1) * nmain * 32 + lane;
+                T v[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) v[j] = j < nmain ? a[j * 32] : (T)0;
+#pragma unroll
+                for (int w = 8; w > 0; w >>= 1)
+#pragma unroll
+                    for (int j = 0; j < w; ++j) v[j] += v[j + w];
+                T sumT = v[0];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sumT += __shfl_xor_sync(0xffffffffu, sumT, o);
+                const double sum = (double)sumT;
+                const double c = p.rho * sum;
+                const bool stop = p.tol > 0.0 && c < p.tol;
+                const bool accept = !stop && c <= thr;
+                const int dec = stop ? 2 : (accept ? 0 : 1);
+                if (lane == 0) {
+                    *reinterpret_cast<volatile int *>(sDec) = dec;
+                    if (p.hist_c && it < p.hist_cap) {
+                        p.hist_c[(size_t)b * p.hist_cap + it] = c; p.hist_a[(size_t)b * p.hist_cap + it] = (unsigned char)accept;
+                    }
+                }
+                c_prev = c_last; c_last = c; thr = p.eta * c; n_it = it + 1;
+                if (accept) ++jacc;
+                else if (!stop) { jacc = 0; ++nrest; }
+                done = stop;
+                return dec;
+            };
+            __syncthreads();
+            int it = 0;
+#pragma unroll 1
+            for (; it < iters; ++it) {
+                __syncthreads();
+                int dec = 0;
+                if (it > 0) dec = decide(it - 1);
+                __syncthreads();
+                if (dec == 2) break;
+                if (dec == 1) { __syncthreads(); __syncthreads(); }
+            }
+            if (!done && iters > 0) { __syncthreads(); decide(iters - 1); __syncthreads(); }
+            if (lane == 0) {
+                InstCtl c = p.ctl[b];
+                c.alpha = alpha_tab[jacc]; c.c_last = c_last;
+                c.c_prev = done ? c_prev : c_last;
+                c.kappa = jacc > 0 ? (double)(T)kappa_tab[jacc - 1] : 0.0;      // momentum of the last hats formed
+                c.done = done ? 1 : 0; c.iters = n_it; c.restarts = nrest;
+                p.ctl[b] = c;
+            }
+            __syncthreads();
+            continue;
+        }
         const int i_cur = p.ctl[b].i_cur;
         const size_t sk = (size_t)b * N + (stage_ok ? k : 0);
         const bool inner = stage_ok && k < N - 1;
@@ -212,14 +302,14 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                             }
                         }
                     }
-                    blk[OG + ((0 * (NXP / 4) + j / 4) * LPS + li) * 4 + (j & 3)] = (T)(p.rho * s0);
-                    blk[OG + ((1 * (NXP / 4) + j / 4) * LPS + li) * 4 + (j & 3)] = (T)(p.rho * s1);
+                    blk[OG + ((0 * (NXP / 2) + j / 2) * LPS + li) * 2 + (j & 1)] = (T)(p.rho * s0);
+                    blk[OG + ((1 * (NXP / 2) + j / 2) * LPS + li) * 2 + (j & 1)] = (T)(p.rho * s1);
                 }
                 if (!GS) {
 #pragma unroll
                     for (int r = 0; r < 2; ++r)
 #pragma unroll
-                        for (int j = 0; j < NXP; ++j) G[r][j % NG] = blk[OG + ((r * (NXP / 4) + j / 4) * LPS + li) * 4 + (j & 3)];
+                        for (int j = 0; j < NXP; ++j) G[r][j % NG] = blk[OG + ((r * (NXP / 2) + j / 2) * LPS + li) * 2 + (j & 1)];
                 }
             }
             sa.z = mk2(st_[0][0], st_[0][1]); sa.v = mk2(st_[1][0], st_[1][1]); sa.th = mk2(st_[2][0], st_[2][1]);
@@ -235,31 +325,18 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             sBnd[2 * ROWP + tid] = (oku0 && DU) ? p.dhi[(size_t)b * p.dbnd_stride + (g0 - nx)] : (T)0;
             sBnd[3 * ROWP + tid] = okr ? p.lo[(size_t)b * p.bnd_stride + g0] : (T)0;
             sBnd[4 * ROWP + tid] = okr ? p.hi[(size_t)b * p.bnd_stride + g0] : (T)0;
-            sBlk[OX + tid] = (tid < NBP && g0 >= 0) ? (tid < NXP ? p.x0[(size_t)b * nx + g0] : p.uprev[(size_t)b * nu + (g0 - nx)]) : (T)0;
+            sBlk[OX + tid] = sBlk[OX + ROWP + tid] =
+                (tid < NBP && g0 >= 0) ? (tid < NXP ? p.x0[(size_t)b * nx + g0] : p.uprev[(size_t)b * nu + (g0 - nx)]) : (T)0;
         }
-        if (tid == 0) { red[32] = p.c0; red[33] = p.c0; sCnt[0] = 0; }
 
-        T kap = (T)0;
-        int jacc = 0, it_done = 0;
-        bool done = false;
-        double *const hc = p.hist_c ? p.hist_c + (size_t)b * p.hist_cap : nullptr;
-        unsigned char *const ha = p.hist_a ? p.hist_a + (size_t)b * p.hist_cap : nullptr;
+        T kap = (T)0;                                          // momentum of the hats being formed
+        int jacc = 0;                                          // accepted steps in a row, the pending one counted as accepted
+        P zh, vh, thh, beh, lah, dh, deh;                      // hats of the iteration in flight (A -> C)
+        P xs, du;                                              // own rows of xbar_{k+1}, Delta u_k of the iteration in flight (B -> C)
+        zh = vh = thh = beh = lah = dh = deh = xs = du = mk2((T)0, (T)0);
 
-        // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the hats overwrite prv's registers, then the new iterate does.
-        // par = it & 1 (compile-time after unrolling by two): c^{i} sits in red[32 + (par ^ 1)], c^{i+1} goes to red[32 + par].
-        auto iteration = [&](R2State<P> &cur, R2State<P> &prv, const int it, const int par) -> bool {
-            // ---- A: steps 6/7 of the previous iteration: hats from (cur, prev, kappa) ----
-            const P kap2 = mk2(kap, kap);
-            const P zh = fma2(kap2, sub2(cur.z, prv.z), cur.z);
-            const P vh = fma2(kap2, sub2(cur.v, prv.v), cur.v);
-            const P thh = fma2(kap2, sub2(cur.th, prv.th), cur.th);
-            const P beh = fma2(kap2, sub2(cur.be, prv.be), cur.be);
-            const P lah = fma2(kap2, sub2(cur.la, prv.la), cur.la);
-            P dh = mk2((T)0, (T)0), deh = dh;
-            if (DU) {
-                dh = fma2(kap2, sub2(cur.d, prv.d), cur.d);
-                deh = fma2(kap2, sub2(cur.de, prv.de), cur.de);
-            }
+        // ---- A: steps 6/7 of the previous iteration: hats from (cur, prev, kappa); publish w, t, rr ----
+        auto publish = [&]() {
             P wv = add2(sub2(zh, vh), lah);                                     // w_k = zhat - vhat - ebar + lambdahat
             if (has_e) wv = sub2(wv, ldp(own + OE));
             P tv = mul2(rho2, sub2(zh, thh));                                   // t_k = rho (zhat - thetahat) [+ qbar]
@@ -267,9 +344,29 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             P rr = sub2(vh, beh);                                               // vhat - betahat [+ dhat - deltahat]
             if (DU) rr = add2(rr, sub2(dh, deh));
             stp(own + OW, wv); stp(own + OT, tv); stp(own + ORR, rr);
-            // (neighbour-to-neighbour mbarrier hand-overs instead of this CTA barrier and the next were measured 12 % slower)
-            __syncthreads();
-            // ---- B: step 1: xbar_{k+1} = Hrow (t + rho [0; w_u]) + G w_x;  Delta u_k = [M B^T | M] rr ----
+        };
+        auto phaseA = [&](const R2State<P> &cur, const R2State<P> &prv) {
+            const P kap2 = mk2(kap, kap);
+            zh = fma2(kap2, sub2(cur.z, prv.z), cur.z);
+            vh = fma2(kap2, sub2(cur.v, prv.v), cur.v);
+            thh = fma2(kap2, sub2(cur.th, prv.th), cur.th);
+            beh = fma2(kap2, sub2(cur.be, prv.be), cur.be);
+            lah = fma2(kap2, sub2(cur.la, prv.la), cur.la);
+            if (DU) {
+                dh = fma2(kap2, sub2(cur.d, prv.d), cur.d);
+                deh = fma2(kap2, sub2(cur.de, prv.de), cur.de);
+            }
+            publish();
+        };
+        // restart (step 7): kappa = 0, hat = the new iterate itself.  Written without the previous iterate ON PURPOSE: it is
+        // then dead from phase A on, and its 14 registers serve phases B and C as load buffers.
+        auto phaseA_restart = [&](const R2State<P> &cur) {
+            zh = cur.z; vh = cur.v; thh = cur.th; beh = cur.be; lah = cur.la;
+            if (DU) { dh = cur.d; deh = cur.de; }
+            publish();
+        };
+        // ---- B: step 1: xbar_{k+1} = Hrow (t + rho [0; w_u]) + G w_x;  Delta u_k = [M B^T | M] rr ----
+        auto phaseB = [&](const int par) {
             P xa[2], da[2];
             xa[0] = xa[1] = da[0] = da[1] = mk2((T)0, (T)0);
 #pragma unroll
@@ -285,8 +382,8 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                     xa[r] = fma2(mk2(Hrow[r][c4 + 2], Hrow[r][c4 + 3]), t1, xa[r]);
                     if (c4 < NXP) {
                         if (GS) {
-                            P g0, g1;
-                            ld4p(blk + OG + ((r * (NXP / 4) + c4 / 4) * LPS + li) * 4, g0, g1);
+                            const P g0 = ldp(blk + OG + ((r * (NXP / 2) + c4 / 2) * LPS + li) * 2);
+                            const P g1 = ldp(blk + OG + ((r * (NXP / 2) + c4 / 2 + 1) * LPS + li) * 2);
                             xa[r] = fma2(g0, w0, xa[r]);
                             xa[r] = fma2(g1, w1, xa[r]);
                         } else {
@@ -298,18 +395,19 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                     da[r] = fma2(mk2(U[r][c4 + 2], U[r][c4 + 3]), r1, da[r]);
                 }
             }
-            const P xs = mk2(xa[0].x + xa[0].y, xa[1].x + xa[1].y);
-            const P du = mk2(da[0].x + da[0].y, da[1].x + da[1].y);              // meaningful on the u rows only
-            stp(own + OX, xs);
-            if (isu) stp(own + ODU - NXP, du);
-            __syncthreads();
-            // ---- C: steps 2-4 ----
+            xs = mk2(xa[0].x + xa[0].y, xa[1].x + xa[1].y);
+            du = mk2(da[0].x + da[0].y, da[1].x + da[1].y);                      // meaningful on the u rows only
+            stp(own + OX + par * ROWP, xs);
+            if (isu) stp(own + ODU + par * NUP - NXP, du);
+        };
+        // ---- C: steps 2-4; the new iterate overwrites prv's registers; the lane's partial of c -> sAcc ----
+        auto phaseC = [&](R2State<P> &prv, const int par) {
             P ba[2], aa[2], xu0 = mk2((T)0, (T)0), xu1 = xu0;
             ba[0] = ba[1] = aa[0] = aa[1] = mk2((T)0, (T)0);
 #pragma unroll
             for (int c4 = 0; c4 < NBP; c4 += 4) {
                 P x0, x1;
-                ld4p(blk - SS + OX + c4, x0, x1);
+                ld4p(blk - SS + OX + par * ROWP + c4, x0, x1);
                 if (NUP == 4 && c4 == NXP) { xu0 = x0; xu1 = x1; }                           // the u part of xbar_k
 #pragma unroll
                 for (int r = 0; r < 2; ++r) {                                               // [A_k B_k] xbar_k (x rows)
@@ -320,7 +418,7 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 #pragma unroll
             for (int c4 = 0; c4 < NUP; c4 += 4) {
                 P u0, u1;
-                ld4p(blk + ODU + c4, u0, u1);
+                ld4p(blk + ODU + par * NUP + c4, u0, u1);
 #pragma unroll
                 for (int r = 0; r < 2; ++r) {                                               // B_k Delta u_k (x rows)
                     aa[r] = fma2(mk2(U[r][NXP + c4], U[r][NXP + c4 + 1]), u0, aa[r]);
@@ -328,7 +426,7 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 }
             }
             // own rows of xbar_k (u rows: the [0 I] rows of Abar_k): with four u rows they sit in the chunk just loaded
-            const P xpi = NUP == 4 ? ((li & 1) ? xu1 : xu0) : ldp(own - SS + OX);
+            const P xpi = NUP == 4 ? ((li & 1) ? xu1 : xu0) : ldp(own - SS + OX + par * ROWP);
             const P a_in = isx ? mk2(aa[0].x + aa[0].y, aa[1].x + aa[1].y) : du;
             P bx = mk2(ba[0].x + ba[0].y, ba[1].x + ba[1].y);
             if (has_e) bx = add2(bx, ldp(own + OE));                                        // pad / u rows hold e = 0
@@ -358,46 +456,54 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 acc2 = fma2(e0, e0, acc2); acc2 = fma2(e1, e1, acc2);
                 prv.d = dn; prv.de = den;
             }
-            // step 4: c = rho * sum (fixed order: group butterfly in T, then double)
-            T acc = acc2.x + acc2.y;
-#pragma unroll
-            for (int o = LPS / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-            double s = (double)acc;
-#pragma unroll
-            for (int o = 16; o >= LPS; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-            if (lane == 0) red[warp] = s;
-            const T kap_acc = jacc < C::KAPN ? sKap[jacc] : (T)kappa_tab[jacc];     // momentum if the step is accepted: off the decision's path
+            // step 4: the lane's partial sum goes to the reducer warp (no shuffles, no fp64 in the stage warps)
+            sAcc[par * nmain * 32 + tid] = acc2.x + acc2.y;
+        };
+        // One iteration of Alg. 1 on (cur, prv) = iterates i, i-1; par = it & 1 (compile-time after unrolling by two).  On
+        // entry phase A of this iteration has run (speculated momentum) and the decision of iteration it-1 is pending
+        // (it > 0): the reducer warp takes it between the two barriers.  Returns true when iteration it-1 stopped (c < tol).
+        auto iteration = [&](R2State<P> &cur, R2State<P> &prv, const int it, const int par) -> bool {
+#ifdef R2_PROF
+            if (blockIdx.x == 0 && lane == 0 && pit < 1024) g_r2prof[(pit * 16 + warp) * 8 + 4] = 0;
+#endif
+            R2P(0);
             __syncthreads();
-            const double c_prev = red[32 + (par ^ 1)];
-            // second level, same bits in every thread: the 16 partials (zeros beyond the CTA's warps), one per lane of each
-            // half-warp, then a four-level butterfly.  Measured on B200 (C4, kernel ms): this 7.95, four partials per lane
-            // + two levels 8.07, sixteen same-address loads + a tree of DADDs 8.13
-            s = red[lane & 15];
-#pragma unroll
-            for (int o = 8; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-            // steps 5-7; every thread decides from the same bits
-            const double c = p.rho * s;
-            it_done = it + 1;
-            const bool stop = p.tol > 0.0 && c < p.tol;
-            const bool accept = !stop && c <= p.eta * c_prev;
-            if (tid == 0) {
-                red[32 + par] = c;
-                if (!accept && !stop) ++sCnt[0];
-                if (hc && it < p.hist_cap) { hc[it] = c; ha[it] = (unsigned char)accept; }
+            R2P(1);
+            phaseB(par);
+            R2P(2);
+            __syncthreads();
+            R2P(3);
+            if (it > 0) {
+                const int dec = *reinterpret_cast<volatile int *>(sDec);       // steps 5-7 of iteration it-1 (the reducer warp)
+                if (dec == 2) return true;
+                if (dec == 1) {                                // restart: A and B again with kappa = 0
+                    kap = (T)0; jacc = 0;
+                    phaseA_restart(cur);
+                    __syncthreads();
+                    phaseB(par);
+                    __syncthreads();
+                    R2P(4);
+                }
             }
-            if (stop) { done = true; return true; }
-            if (accept) {
-                kap = kap_acc;
-                ++jacc;
-            } else {
-                kap = (T)0; jacc = 0;
-            }
+            phaseC(prv, par);
+            T kg = (T)0;
+            if (jacc >= C::KAPN) kg = (T)kappa_tab[jacc];
+            kap = jacc < C::KAPN ? sKap[jacc] : kg;            // speculate: the step is accepted
+            ++jacc;
+            phaseA(prv, cur);                                  // hats of iteration it + 1: the new iterate sits in prv's registers
+            R2P(5);
+#ifdef R2_PROF
+            ++pit;
+#endif
             return false;
         };
 
         // ---- results: iterate -> S[i_cur], xbar and Delta u of the last iteration (called at each exit of the loop: the
-        // two iterate sets never merge, so the unrolled-by-two loop carries them in place without register moves) ----
-        auto write_back = [&](const R2State<P> &fin) {
+        // two iterate sets never merge, so the unrolled-by-two loop carries them in place without register moves).
+        // the last iteration had parity par; pending: its decision is still open (the reducer warp takes it between two barriers) ----
+        auto finish = [&](const R2State<P> &fin, const bool pending, const int par) {
+            if (pending) { __syncthreads(); __syncthreads(); }
+            const size_t sk = (size_t)b * N + (stage_ok ? k : 0);
             const T fz[2] = {fin.z.x, fin.z.y}, fv[2] = {fin.v.x, fin.v.y}, fth[2] = {fin.th.x, fin.th.y};
             const T fbe[2] = {fin.be.x, fin.be.y}, fla[2] = {fin.la.x, fin.la.y}, fd[2] = {fin.d.x, fin.d.y}, fde[2] = {fin.de.x, fin.de.y};
 #pragma unroll
@@ -407,9 +513,9 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                     T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(b, k);
                     rec[p.oZ() + gi] = fz[r]; rec[p.oV() + gi] = fv[r]; rec[p.oTH() + gi] = fth[r];
                     rec[p.oBE() + gi] = fbe[r]; rec[p.oLA() + gi] = fla[r];
-                    p.X[sk * nb + gi] = own[OX + r];
+                    p.X[sk * nb + gi] = own[OX + par * ROWP + r];
                     if (i0 >= NXP) {
-                        p.DU[sk * nu + (gi - nx)] = own[ODU - NXP + r];
+                        p.DU[sk * nu + (gi - nx)] = own[ODU + par * NUP - NXP + r];
                         if (DU) { rec[p.oD() + (gi - nx)] = fd[r]; rec[p.oDE() + (gi - nx)] = fde[r]; }
                     }
                 }
@@ -417,26 +523,40 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         };
 
         __syncthreads();
+#ifdef R2_PROF
+        pit = 0; R2P(5); pit = 1;
+#endif
+        phaseA(sa, sb);                                        // kappa = 0: hats = iterates (Alg. 1 input)
         {
             int it = 0;
+#pragma unroll 1
             for (;;) {
-                if (it >= iters) { write_back(sa); break; }
-                if (iteration(sa, sb, it, 0) || it + 1 >= iters) { write_back(sb); break; }
-                if (iteration(sb, sa, it + 1, 1)) { write_back(sa); break; }
+                if (it >= iters) { finish(sa, it > 0, 1); break; }
+                if (iteration(sa, sb, it, 0)) { finish(sa, false, 1); break; }           // iteration it-1 stopped
+                if (it + 1 >= iters) { finish(sb, true, 0); break; }
+                if (iteration(sb, sa, it + 1, 1)) { finish(sb, false, 0); break; }       // iteration it stopped
                 it += 2;
             }
         }
-        __syncthreads();                         // red[], sCnt of the last iteration are visible to thread 0
-        if (tid == 0) {
-            InstCtl c = p.ctl[b];
-            const int last = (it_done - 1) & 1;
-            c.alpha = alpha_tab[jacc]; c.c_last = it_done ? red[32 + last] : p.c0;
-            c.c_prev = done ? red[32 + (last ^ 1)] : c.c_last;
-            c.kappa = (double)kap;
-            c.done = done ? 1 : 0; c.iters = it_done; c.restarts = sCnt[0];
-            p.ctl[b] = c;
-        }
         __syncthreads();
+#ifdef R2_PROF
+        if (blockIdx.x == 0 && b == 0 && lane == 0 && (warp == 0 || warp == nmain - 1 || warp == 5)) {
+            // slots: 0 after A, 1 after bar1, 2 after B, 3 after bar2, 4 redo (A and B again), 5 after C; row pit-1 slot 5/4 = start
+            // slots: 0 at entry (after C + A of the previous iteration), 1 after bar1, 2 after B, 3 after bar2, 4 after a redo, 5 end
+            long long acc[6] = {0, 0, 0, 0, 0, 0};
+            int nredo = 0;
+            for (int r = 1; r < pit && r < 1024; ++r) {
+                const long long *cur = g_r2prof + (r * 16 + warp) * 8, *prv = g_r2prof + ((r - 1) * 16 + warp) * 8;
+                acc[0] += cur[0] - prv[5]; acc[1] += cur[1] - cur[0]; acc[2] += cur[2] - cur[1]; acc[3] += cur[3] - cur[2];
+                long long t3 = cur[3];
+                if (cur[4] > cur[3]) { acc[4] += cur[4] - cur[3]; t3 = cur[4]; ++nredo; }
+                acc[5] += cur[5] - t3;
+            }
+            printf("R2_PROF warp %d iters %d redo %d: gap %lld bar1 %lld B %lld bar2 %lld redo(A,B) %lld C+A %lld  total %lld (cycles per iteration)\n",
+                   warp, iters, nredo, acc[0] / iters, acc[1] / iters, acc[2] / iters, acc[3] / iters, acc[4] / iters, acc[5] / iters,
+                   (acc[0] + acc[1] + acc[2] + acc[3] + acc[4] + acc[5]) / iters);
+        }
+#endif
     }
 }
 
@@ -444,31 +564,32 @@ template <typename T, int NXP, int NUP, int MAXT, bool GS>
 int launch_res2(pimpc_s *h, int iters, double tol)
 {
     using C = R2Cfg<T, NXP, NUP, GS>;
-    const int nwarps = (h->N + C::SPW - 1) / C::SPW;
+    const int nmain = (h->N + C::SPW - 1) / C::SPW, nthr = (nmain + 1) * 32;   // stage warps + the reducer warp
     auto kern = h->has_du ? k_res2<T, NXP, NUP, MAXT, true, GS> : k_res2<T, NXP, NUP, MAXT, false, GS>;
-    const size_t smem = C::smem_bytes(nwarps);
+    const size_t smem = C::smem_bytes(nmain);
     PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    PIMPC_CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nwarps * 32, smem));
-    if (occ < 1) { h->errmsg = "RESIDENT kernel does not fit on an SM"; return PIMPC_EINVAL; }
+    PIMPC_CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nthr, smem));
+    if (occ < 1 || nthr > MAXT) { h->errmsg = "RESIDENT kernel does not fit on an SM"; return PIMPC_EINVAL; }
     const int grid = std::min(h->batch, h->sm_count * occ);
     Prob<T> p = make_prob<T>(h, tol);
-    kern<<<grid, nwarps * 32, smem, h->stream>>>(p, h->alpha_tab, h->kappa_tab, iters);
+    kern<<<grid, nthr, smem, h->stream>>>(p, h->alpha_tab, h->kappa_tab, iters);
     PIMPC_CUDA_TRY(h, cudaGetLastError());
-    h->info.grid = grid; h->info.block = nwarps * 32; h->info.smem_bytes = smem;
+    h->info.grid = grid; h->info.block = nthr; h->info.smem_bytes = smem;
     return 1;
 }
 
 } // namespace
 
-// Padded shapes with an instantiation, smallest first: {NXP, NUP, stages per warp, max warps}.  fp32 keeps 2 * (2 NBP + NXP)
-// matrix words per lane in registers (88 for (12, 4)) while the CTA has at most 12 warps (168 registers per thread);
-// 13..16 warps (128 registers) move the 2 NXP words of G_k to shared memory.  fp64 doubles the words: (4, 4) only.
+// Padded shapes with an instantiation, smallest first: {NXP, NUP, stages per warp, max STAGE warps}; the CTA has one more
+// warp, the reducer.  fp32 keeps 2 * (2 NBP + NXP) matrix words per lane in registers (88 for (12, 4)) while the CTA has at
+// most 12 warps (168 registers per thread); 13..16 warps (128 registers) move the 2 NXP words of G_k to shared memory.
+// fp64 doubles the words: (4, 4) only.
 bool resident2_plan(const pimpc_s *h, int *nxp, int *nup, int *maxn)
 {
     struct S { int nxp, nup, spw, maxw; };
-    static const S f32[] = {{4, 4, 8, 16}, {8, 4, 4, 16}, {8, 8, 4, 16}, {12, 4, 4, 16}};
-    static const S f64[] = {{4, 4, 8, 8}};
+    static const S f32[] = {{4, 4, 8, 15}, {8, 4, 4, 15}, {8, 8, 4, 15}, {12, 4, 4, 15}};
+    static const S f64[] = {{4, 4, 8, 7}};
     const S *tab = h->dtype == PIMPC_F32 ? f32 : f64;
     const int n = h->dtype == PIMPC_F32 ? 4 : 1;
     for (int i = 0; i < n; ++i)
@@ -486,7 +607,7 @@ int run_resident2(pimpc_s *h, int iters, double tol)
     if (h->dtype == PIMPC_F64) return launch_res2<double, 4, 4, 256, false>(h, iters, tol);
     if (nxp == 4) return launch_res2<float, 4, 4, 512, false>(h, iters, tol);
     if (nxp == 8 && nup == 4) return launch_res2<float, 8, 4, 512, false>(h, iters, tol);
-    const bool small = h->N <= 48;                             // <= 12 warps of 4 stages
+    const bool small = h->N <= 44;                             // <= 11 stage warps of 4 stages + the reducer: 12 warps
     if (nxp == 8) return small ? launch_res2<float, 8, 8, 384, false>(h, iters, tol) : launch_res2<float, 8, 8, 512, true>(h, iters, tol);
     return small ? launch_res2<float, 12, 4, 384, false>(h, iters, tol) : launch_res2<float, 12, 4, 512, true>(h, iters, tol);
 }
