@@ -46,17 +46,10 @@ template <> struct Pr<double> { typedef double2 t; };
 
 __device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
-#ifdef R2_SCALAR
-__device__ __forceinline__ float2 add2(float2 a, float2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
-__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
-__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return make_float2(__fmaf_rn(a.x, b.x, c.x), __fmaf_rn(a.y, b.y, c.y)); }
-__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return make_float2(__fsub_rn(a.x, b.x), __fsub_rn(a.y, b.y)); }
-#else
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }   // a - b, one rounding
-#endif
 __device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 mul2(double2 a, double2 b) { return make_double2(a.x * b.x, a.y * b.y); }
 __device__ __forceinline__ double2 fma2(double2 a, double2 b, double2 c) { return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
@@ -369,31 +362,43 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         auto phaseB = [&](const int par) {
             P xa[2], da[2];
             xa[0] = xa[1] = da[0] = da[1] = mk2((T)0, (T)0);
+            // one vector at a time, all its chunks in flight before its products (with the three vectors interleaved chunk by
+            // chunk ptxas sank every load next to its use, and the in-order warp paid the 29-cycle shared-memory latency
+            // once per chunk: C4 kernel 7.37 -> 7.09 ms): t, then rr, then w -- the u part of w first, it joins t (the
+            // [0 I] rows of Abar_{k+1})
+            P tv[NBP / 2], wv[NBP / 2];
 #pragma unroll
-            for (int c4 = 0; c4 < NBP; c4 += 4) {
-                P t0, t1, w0, w1, r0, r1;
-                ld4p(blk + OT + c4, t0, t1);
-                ld4p(blk + SS + OW + c4, w0, w1);
-                ld4p(blk + ORR + c4, r0, r1);
-                if (c4 >= NXP) { t0 = fma2(rho2, w0, t0); t1 = fma2(rho2, w1, t1); }       // the [0 I] rows of Abar_{k+1}
+            for (int c4 = NXP; c4 < NBP; c4 += 4) ld4p(blk + SS + OW + c4, wv[c4 / 2], wv[c4 / 2 + 1]);
+#pragma unroll
+            for (int c4 = 0; c4 < NBP; c4 += 4) ld4p(blk + OT + c4, tv[c4 / 2], tv[c4 / 2 + 1]);
+#pragma unroll
+            for (int c2 = NXP / 2; c2 < NBP / 2; ++c2) tv[c2] = fma2(rho2, wv[c2], tv[c2]);
+#pragma unroll
+            for (int c2 = 0; c2 < NBP / 2; ++c2)
+#pragma unroll
+                for (int r = 0; r < 2; ++r) xa[r] = fma2(mk2(Hrow[r][2 * c2], Hrow[r][2 * c2 + 1]), tv[c2], xa[r]);
+#pragma unroll
+            for (int c4 = 0; c4 < NBP; c4 += 4) ld4p(blk + ORR + c4, tv[c4 / 2], tv[c4 / 2 + 1]);
+#pragma unroll
+            for (int c4 = 0; c4 < NXP; c4 += 4) ld4p(blk + SS + OW + c4, wv[c4 / 2], wv[c4 / 2 + 1]);
+#pragma unroll
+            for (int c2 = 0; c2 < NBP / 2; ++c2)
+#pragma unroll
+                for (int r = 0; r < 2; ++r) da[r] = fma2(mk2(U[r][2 * c2], U[r][2 * c2 + 1]), tv[c2], da[r]);
+            if (GS) {                                          // the rows of G_k from shared memory, a row's pieces in flight together
 #pragma unroll
                 for (int r = 0; r < 2; ++r) {
-                    xa[r] = fma2(mk2(Hrow[r][c4], Hrow[r][c4 + 1]), t0, xa[r]);
-                    xa[r] = fma2(mk2(Hrow[r][c4 + 2], Hrow[r][c4 + 3]), t1, xa[r]);
-                    if (c4 < NXP) {
-                        if (GS) {
-                            const P g0 = ldp(blk + OG + ((r * (NXP / 2) + c4 / 2) * LPS + li) * 2);
-                            const P g1 = ldp(blk + OG + ((r * (NXP / 2) + c4 / 2 + 1) * LPS + li) * 2);
-                            xa[r] = fma2(g0, w0, xa[r]);
-                            xa[r] = fma2(g1, w1, xa[r]);
-                        } else {
-                            xa[r] = fma2(mk2(G[r][c4 % NG], G[r][(c4 + 1) % NG]), w0, xa[r]);
-                            xa[r] = fma2(mk2(G[r][(c4 + 2) % NG], G[r][(c4 + 3) % NG]), w1, xa[r]);
-                        }
-                    }
-                    da[r] = fma2(mk2(U[r][c4], U[r][c4 + 1]), r0, da[r]);
-                    da[r] = fma2(mk2(U[r][c4 + 2], U[r][c4 + 3]), r1, da[r]);
+                    P g[NXP / 2];
+#pragma unroll
+                    for (int c2 = 0; c2 < NXP / 2; ++c2) g[c2] = ldp(blk + OG + ((r * (NXP / 2) + c2) * LPS + li) * 2);
+#pragma unroll
+                    for (int c2 = 0; c2 < NXP / 2; ++c2) xa[r] = fma2(g[c2], wv[c2], xa[r]);
                 }
+            } else {
+#pragma unroll
+                for (int c2 = 0; c2 < NXP / 2; ++c2)
+#pragma unroll
+                    for (int r = 0; r < 2; ++r) xa[r] = fma2(mk2(G[r][(2 * c2) % NG], G[r][(2 * c2 + 1) % NG]), wv[c2], xa[r]);
             }
             xs = mk2(xa[0].x + xa[0].y, xa[1].x + xa[1].y);
             du = mk2(da[0].x + da[0].y, da[1].x + da[1].y);                      // meaningful on the u rows only
