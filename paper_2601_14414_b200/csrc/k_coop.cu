@@ -164,7 +164,9 @@ struct OCfg {
     // one block per virtual slot v = 0..L+1 (stage k0 - 1 + v):
     //   W w_k = zhat - vhat - ebar + lambdahat   X xbar_{k+1}   D vhat - betahat   HH h_k   RH rhs of the Delta-u update
     //   DU Delta u_k   E e_k   HM H_k [NB][HS]   AB [A_k B_k] [NX][HS]   MM M_k [NU][NUP]
-    static constexpr int OW = 0, OX = LPS, OD = 2 * LPS, OHH = 3 * LPS, ORH = 4 * LPS, ODU = ORH + NUP, OE = ODU + NUP,
+    // X and DU exist twice (parity of the iteration: the speculated phases B, C of the next iteration must not destroy the
+    // primal step of an iteration that turns out to have stopped): OX + par * LPS, ODU + par * NUP
+    static constexpr int OW = 0, OX = LPS, OD = 3 * LPS, OHH = 4 * LPS, ORH = 5 * LPS, ODU = ORH + NUP, OE = ODU + 2 * NUP,
                          OHM = OE + LPS, OAB = OHM + NB * HS, OMM = OAB + NX * HS, SS0 = OMM + NU * NUP;
     // slot stride == LPS words (mod 32): the groups of a warp work on consecutive slots and hit disjoint banks
     static constexpr int SSW0 = SS0 * WPE;
@@ -176,7 +178,8 @@ struct OCfg {
     static constexpr int CLMAX = 16;
     static constexpr size_t xpart_bytes = 2 * CLMAX * 16, xhalo_bytes = 2 * 5 * LPS * 4 * sizeof(T);
     static constexpr size_t head_bytes = 40 * sizeof(double) + xpart_bytes + xhalo_bytes + (KAPN + 2 * LPS + 2 * NUP) * sizeof(T);
-    static size_t smem_bytes(int slots) { return head_bytes + (size_t)slots * SS * sizeof(T); }
+    // + [2][threads] per-lane partial sums of c (by parity of the iteration), behind the slots
+    static size_t smem_bytes(int slots, int threads) { return head_bytes + ((size_t)slots * SS + 2 * (size_t)threads) * sizeof(T); }
     // exchange buffers per CTA and parity (tagged words): to the left neighbour (z, v, lambda) of the first stage,
     // to the right neighbour (z, theta) of the last stage
     static constexpr int HALO = 5 * LPS;
@@ -191,7 +194,7 @@ template <typename T> struct OState { T z, v, th, be, la, d, de; };
 template <typename T, int NX, int NU, int SPG, int MAXT, bool DU, bool CL>
 __global__ void __launch_bounds__(MAXT, 1)
 k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__restrict__ kappa_tab, const int iters,
-       typename Tagged<double>::W *__restrict__ part, typename Tagged<T>::W *__restrict__ halo)
+       typename Tagged<double>::W *__restrict__ part, typename Tagged<T>::W *__restrict__ halo, const int spec)
 {
     using C = OCfg<T, NX, NU>;
     using TW = Tagged<T>;
@@ -232,7 +235,6 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         sDlo[tid] = (DU && tid < nu) ? p.dlo[tid] : (T)0;
         sDhi[tid] = (DU && tid < nu) ? p.dhi[tid] : (T)0;
     }
-    if (tid == 0) { red[32] = p.c0; red[33] = p.c0; }
     if (CL) {
         for (int i = tid; i < (int)((C::xpart_bytes + C::xhalo_bytes) / 4); i += blockDim.x) reinterpret_cast<uint32_t *>(xPart)[i] = 0u;
     }
@@ -263,7 +265,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     }
     if (!has_left && tid < LPS) {                              // slot 0 of the first CTA: xbar_0 = (x(t); u(t-1))
         const int g0 = tid < NB ? gidx(tid) : -1;
-        sBlk[OX + tid] = g0 < 0 ? (T)0 : (tid < NX ? p.x0[g0] : p.uprev[g0 - nx]);
+        sBlk[OX + tid] = sBlk[OX + LPS + tid] = g0 < 0 ? (T)0 : (tid < NX ? p.x0[g0] : p.uprev[g0 - nx]);
     }
 
     OState<T> sa[SPG], sb[SPG];
@@ -297,18 +299,36 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     const int mrow = (li >= NX && rowok) ? li - NX : 0;
     const bool ulane = li >= NX && rowok;
 
-    T kap = (T)0;
-    int jacc = 0, it_done = 0, restarts = 0;
-    bool done = false;
+    T kap = (T)0;                                // momentum of the hats being formed
+    int jacc = 0;                                // accepted steps in a row, a pending (speculated) one counted as accepted
     unsigned long long xold[2][3] = {{0ull, 0ull, 0ull}, {0ull, 0ull, 0ull}};     // this CTA's limbs still inside the two parity slots
+    // the accept / restart state of Alg. 1 lives in shared memory (lane 0 of the communication warp reads and writes it):
+    // red[32] = c of the last iteration, red[33] = c of the one before; sCtl = {accepted steps in a row, restarts, iterations, done}
+    int *sCtl = reinterpret_cast<int *>(red + 36);
+    if (tid == 0) { red[32] = p.c0; red[33] = p.c0; sCtl[0] = sCtl[1] = sCtl[2] = sCtl[3] = 0; }
+    const int slots_max = (N + G - 1) / G + 2;
+    T *sAcc = sBlk + (size_t)slots_max * SS;     // [2][blockDim.x] per-lane partial sums of c by parity of the iteration
+    int *sDec = reinterpret_cast<int *>(red + 34);   // decision of the communication warp: 0 accept, 1 restart, 2 stop
     __syncthreads();
     if (CL) cluster_sync_all();                  // every CTA of the cluster has zeroed its inbound words
 
-    // One iteration of Alg. 1.  cur/prv: iterate i and i-1; the new iterate overwrites prv.  par = it & 1.
-    auto iteration = [&](OState<T> (&cur)[SPG], OState<T> (&prv)[SPG], const int it, const int par) -> bool {
-        const uint32_t tag = (uint32_t)it + 1u;
-        T zh[SPG], vh[SPG], thh[SPG], beh[SPG], lah[SPG], dh[SPG], deh[SPG], dv[SPG], ev[SPG];
-        // ---- A: steps 6/7 of the previous iteration: hats from (cur, prev, kappa); w, vhat - betahat ----
+    T zh[SPG], vh[SPG], thh[SPG], beh[SPG], lah[SPG], dh[SPG], deh[SPG], dv[SPG], ev[SPG];   // hats of the iteration in flight
+    T xs[SPG], du[SPG];                                                                    // its primal step (own rows)
+#pragma unroll
+    for (int s = 0; s < SPG; ++s) { zh[s] = vh[s] = thh[s] = beh[s] = lah[s] = dh[s] = deh[s] = dv[s] = ev[s] = xs[s] = du[s] = (T)0; }
+
+    // ---- A: steps 6/7 of the previous iteration: hats from (cur, prev, kappa); publish w, vhat - betahat ----
+    auto publish = [&]() {
+#pragma unroll
+        for (int s = 0; s < SPG; ++s) {
+            dv[s] = vh[s] - beh[s];
+            T w = zh[s] - vh[s] + lah[s];
+            ev[s] = (T)0;
+            if (has_e && exist[s]) { ev[s] = blkp[s][OE + li]; w -= ev[s]; }
+            if (exist[s]) { blkp[s][OW + li] = w; blkp[s][OD + li] = dv[s]; }
+        }
+    };
+    auto phaseA = [&](OState<T> (&cur)[SPG], OState<T> (&prv)[SPG]) {
 #pragma unroll
         for (int s = 0; s < SPG; ++s) {
             zh[s] = cur[s].z + kap * (cur[s].z - prv[s].z);
@@ -320,14 +340,21 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 dh[s] = cur[s].d + kap * (cur[s].d - prv[s].d);
                 deh[s] = cur[s].de + kap * (cur[s].de - prv[s].de);
             }
-            dv[s] = vh[s] - beh[s];
-            T w = zh[s] - vh[s] + lah[s];
-            ev[s] = (T)0;
-            if (has_e && exist[s]) { ev[s] = blkp[s][OE + li]; w -= ev[s]; }
-            if (exist[s]) { blkp[s][OW + li] = w; blkp[s][OD + li] = dv[s]; }
         }
-        __syncthreads();
-        // ---- B: step 1: g = Abar_{k+1}^T w_{k+1}, h_k; rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat] ----
+        publish();
+    };
+    // restart (step 7): kappa = 0, hat = the new iterate itself (the previous iterate is not needed)
+    auto phaseA_restart = [&](OState<T> (&cur)[SPG]) {
+#pragma unroll
+        for (int s = 0; s < SPG; ++s) {
+            zh[s] = cur[s].z; vh[s] = cur[s].v; thh[s] = cur[s].th; beh[s] = cur[s].be; lah[s] = cur[s].la;
+            if (DU) { dh[s] = cur[s].d; deh[s] = cur[s].de; }
+        }
+        publish();
+    };
+    // ---- B, C: step 1 ----
+    auto phaseBC = [&](const int par) {
+        // B: g = Abar_{k+1}^T w_{k+1}, h_k; rhs = Bbar_k^T (vhat - betahat) [+ dhat - deltahat]
 #pragma unroll
         for (int s = 0; s < SPG; ++s) {
             if (!(real[s] || ghl[s])) continue;
@@ -356,8 +383,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             if (ulane) blkp[s][ORH + li - NX] = rr;
         }
         __syncwarp();
-        // ---- C: xbar_{k+1} = H_k h_k; Delta u_k = M_k rhs ----
-        T xs[SPG], du[SPG];
+        // C: xbar_{k+1} = H_k h_k; Delta u_k = M_k rhs
 #pragma unroll
         for (int s = 0; s < SPG; ++s) {
             xs[s] = (T)0; du[s] = (T)0;
@@ -372,7 +398,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 x0 += m4[0] * h4[0]; x1 += m4[1] * h4[1]; x0 += m4[2] * h4[2]; x1 += m4[3] * h4[3];
             }
             xs[s] = rowok ? x0 + x1 : (T)0;
-            blkp[s][OX + li] = xs[s];
+            blkp[s][OX + par * LPS + li] = xs[s];
             if (real[s]) {
                 T d0 = (T)0;
 #pragma unroll
@@ -384,11 +410,14 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                     for (int q = 0; q < 4; ++q) d0 += m4[q] * r4[q];
                 }
                 du[s] = ulane ? d0 : (T)0;
-                if (ulane) blkp[s][ODU + li - NX] = du[s];
+                if (ulane) blkp[s][ODU + par * NUP + li - NX] = du[s];
             }
         }
-        __syncthreads();
-        // ---- D: steps 2-4 of the real stages ----
+    };
+    // ---- D: steps 2-4 of the real stages; the new iterate overwrites prv; boundary iterates to the
+    // neighbours; this lane's partial sum of c to the communication warp ----
+    auto phaseD = [&](OState<T> (&prv)[SPG], const int it, const int par) {
+        const uint32_t tag = (uint32_t)it + 1u;
         T acc = (T)0;
 #pragma unroll
         for (int s = 0; s < SPG; ++s) {
@@ -398,18 +427,18 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 #pragma unroll
             for (int c4 = 0; c4 < NBP; c4 += 4) {
                 T x4[4], a4[4];
-                ld4o(prvb + OX + c4, x4);
+                ld4o(prvb + OX + par * LPS + c4, x4);
                 ld4o(blk + OAB + xrow * HS + c4, a4);
                 t0 += a4[0] * x4[0]; t1 += a4[1] * x4[1]; t0 += a4[2] * x4[2]; t1 += a4[3] * x4[3];   // [A_k B_k] xbar_k (x-rows)
                 if (c4 >= NX) {
                     T u4[4];
-                    ld4o(blk + ODU + (c4 - NX), u4);
+                    ld4o(blk + ODU + par * NUP + (c4 - NX), u4);
 #pragma unroll
                     for (int q = 0; q < 4; ++q) avx += a4[q] * u4[q];                                  // B_k Delta u_k (x-rows)
                 }
             }
             const bool xr = li < NX;
-            const T xpi = prvb[OX + li];
+            const T xpi = prvb[OX + par * LPS + li];
             const T duu = isx ? (T)0 : du[s];
             const T av = (isx ? (xr ? avx : (T)0) : du[s]) + beh[s];                    // a = Bbar du + betahat
             const T bv = (isx ? (xr ? t0 + t1 + ev[s] : (T)0) : xpi) - lah[s];          // b = Abar xbar_k + ebar - lambdahat
@@ -451,121 +480,196 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 }
             }
         }
-        // ---- step 4: c = rho * sum (fixed order: group butterfly in T, then double) ----
+        sAcc[par * blockDim.x + tid] = acc;                                    // (communication warp: zero)
+    };
+    // ---- the ghosts' new iterates, published by the neighbours in their phase D of iteration `it` ----
+    auto ghosts = [&](OState<T> (&prv)[SPG], const int it, const int par) {
+        const uint32_t tag = (uint32_t)it + 1u;
 #pragma unroll
-        for (int o = LPS / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        double sum = (double)acc;
+        for (int s = 0; s < SPG; ++s) {
+            if (ghl[s] && rowok) {
+                const typename TW::W *o = CL ? xHalo + par * C::HALO + 3 * LPS : halo + ((size_t)par * G + cta - 1) * C::HALO + 3 * LPS;
+                T a, b2;
+                bool ga = false, gb = false;
+                do {
+                    if (!ga) ga = CL ? TW::ld_sm(o + li, tag, a) : TW::ld(o + li, tag, a);
+                    if (!gb) gb = CL ? TW::ld_sm(o + LPS + li, tag, b2) : TW::ld(o + LPS + li, tag, b2);
+                } while (!(ga && gb));
+                prv[s].z = a; prv[s].th = b2;
+            }
+            if (ghr[s] && rowok) {
+                const typename TW::W *o = CL ? xHalo + par * C::HALO : halo + ((size_t)par * G + cta + 1) * C::HALO;
+                T a, b2, c2;
+                bool ga = false, gb = false, gc = false;
+                do {
+                    if (!ga) ga = CL ? TW::ld_sm(o + li, tag, a) : TW::ld(o + li, tag, a);
+                    if (!gb) gb = CL ? TW::ld_sm(o + LPS + li, tag, b2) : TW::ld(o + LPS + li, tag, b2);
+                    if (!gc) gc = CL ? TW::ld_sm(o + 2 * LPS + li, tag, c2) : TW::ld(o + 2 * LPS + li, tag, c2);
+                } while (!(ga && gb && gc));
+                prv[s].z = a; prv[s].v = b2; prv[s].la = c2;
+            }
+        }
+    };
+    // ---- communication warp: step 4 (the sum over the CTA, then over the CTAs) and steps 5-7 of iteration
+    // `it`; publishes the decision to the compute warps.  Called between two CTA barriers, after every lane's phase D ----
+    auto decide = [&](const int it) {
+        if (!comm) return;
+        const int par = it & 1;
+        const uint32_t tag = (uint32_t)it + 1u;
+        // fixed order: this lane's column over the compute warps (loads in flight together, a balanced tree in T), the butterfly
+        // over the lanes, then double
+        const T *a = sAcc + par * blockDim.x + lane;
+        T sT = (T)0;
 #pragma unroll
-        for (int o = 16; o >= LPS; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-        if (lane == 0 && !comm) red[warp] = sum;
-        __syncthreads();
-        if (comm) {
-            sum = lane < ncw ? red[lane] : 0.0;
+        for (int j0 = 0; j0 < 32; j0 += 8) {                   // eight warps at a time (register budget of the 1024-thread variants)
+            T v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) v[j] = j0 + j < ncw ? a[(j0 + j) * 32] : (T)0;
+#pragma unroll
+            for (int w = 4; w > 0; w >>= 1)
+#pragma unroll
+                for (int j = 0; j < w; ++j) v[j] += v[j + w];
+            sT += v[0];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sT += __shfl_xor_sync(0xffffffffu, sT, o);
+        double sum = (double)sT;
+        if (CL) {                                  // push the partial into every CTA of the cluster, poll the own copies
+            if (lane < G) TD::st_cl(map_peer(xPart + par * C::CLMAX + cta, lane), sum, tag);
+            double val = 0.0;
+            if (lane < G) while (!TD::ld_sm(xPart + par * C::CLMAX + lane, tag, val)) {}
+            sum = val;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            if (CL) {                                  // push the partial into every CTA of the cluster, poll the own copies
-                if (lane < G) TD::st_cl(map_peer(xPart + par * C::CLMAX + cta, lane), sum, tag);
-                double val = 0.0;
-                if (lane < G) while (!TD::ld_sm(xPart + par * C::CLMAX + lane, tag, val)) {}
-                sum = val;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            } else {
-                // exact fixed-point atomic sum (see to_limbs): parity slot, three adjacent words, never reset
-                unsigned long long *acc = reinterpret_cast<unsigned long long *>(part) + (size_t)par * 32;
-                if (lane == 0) {
-                    const Limbs L = to_limbs(sum);
-                    const unsigned expect = (unsigned)((it / 2 + 1) * G) & 255u;              // arrivals in this slot so far, mod 256
-                    const unsigned long long one = 1ull << 56, mask = one - 1;
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) {
-                        red_add_relaxed(acc + q, L.l[q] - xold[par][q] + one);
-                        xold[par][q] = L.l[q];
-                    }
-                    unsigned long long v0, v1, v2;
-                    do {
-                        v0 = ld_relaxed(acc); v1 = ld_relaxed(acc + 1); v2 = ld_relaxed(acc + 2);
-                    } while ((unsigned)(v0 >> 56) != expect || (unsigned)(v1 >> 56) != expect || (unsigned)(v2 >> 56) != expect);
-                    sum = from_limbs(v0 & mask, v1 & mask, v2 & mask);
-                }
-                sum = __shfl_sync(0xffffffffu, sum, 0);
-            }
-            if (lane == 0) red[32 + par] = p.rho * sum;
         } else {
-            // the ghosts' new iterates, published by the neighbours in their phase D of this iteration
+            // exact fixed-point atomic sum (see to_limbs): parity slot, three adjacent words, never reset
+            unsigned long long *acc = reinterpret_cast<unsigned long long *>(part) + (size_t)par * 32;
+            if (lane == 0) {
+                const Limbs Lm = to_limbs(sum);
+                const unsigned expect = (unsigned)((it / 2 + 1) * G) & 255u;              // arrivals in this slot so far, mod 256
+                const unsigned long long one = 1ull << 56, mask = one - 1;
 #pragma unroll
-            for (int s = 0; s < SPG; ++s) {
-                if (ghl[s] && rowok) {
-                    const typename TW::W *o = CL ? xHalo + par * C::HALO + 3 * LPS : halo + ((size_t)par * G + cta - 1) * C::HALO + 3 * LPS;
-                    T a, b2;
-                    bool ga = false, gb = false;
-                    do {
-                        if (!ga) ga = CL ? TW::ld_sm(o + li, tag, a) : TW::ld(o + li, tag, a);
-                        if (!gb) gb = CL ? TW::ld_sm(o + LPS + li, tag, b2) : TW::ld(o + LPS + li, tag, b2);
-                    } while (!(ga && gb));
-                    prv[s].z = a; prv[s].th = b2;
+                for (int q = 0; q < 3; ++q) {
+                    red_add_relaxed(acc + q, Lm.l[q] - xold[par][q] + one);
+                    xold[par][q] = Lm.l[q];
                 }
-                if (ghr[s] && rowok) {
-                    const typename TW::W *o = CL ? xHalo + par * C::HALO : halo + ((size_t)par * G + cta + 1) * C::HALO;
-                    T a, b2, c2;
-                    bool ga = false, gb = false, gc = false;
-                    do {
-                        if (!ga) ga = CL ? TW::ld_sm(o + li, tag, a) : TW::ld(o + li, tag, a);
-                        if (!gb) gb = CL ? TW::ld_sm(o + LPS + li, tag, b2) : TW::ld(o + LPS + li, tag, b2);
-                        if (!gc) gc = CL ? TW::ld_sm(o + 2 * LPS + li, tag, c2) : TW::ld(o + 2 * LPS + li, tag, c2);
-                    } while (!(ga && gb && gc));
-                    prv[s].z = a; prv[s].v = b2; prv[s].la = c2;
-                }
+                unsigned long long v0, v1, v2;
+                do {
+                    v0 = ld_relaxed(acc); v1 = ld_relaxed(acc + 1); v2 = ld_relaxed(acc + 2);
+                } while ((unsigned)(v0 >> 56) != expect || (unsigned)(v1 >> 56) != expect || (unsigned)(v2 >> 56) != expect);
+                sum = from_limbs(v0 & mask, v1 & mask, v2 & mask);
             }
+            sum = __shfl_sync(0xffffffffu, sum, 0);
         }
-        __syncthreads();
-        // ---- steps 5-7; every thread of every CTA decides from the same bits ----
-        const double c = red[32 + par], c_prev = red[32 + (par ^ 1)];
-        it_done = it + 1;
-        const bool stop = p.tol > 0.0 && c < p.tol;
-        const bool accept = !stop && c <= p.eta * c_prev;
-        if (!accept && !stop) ++restarts;
-        if (cta == 0 && tid == 0 && p.hist_c && it < p.hist_cap) { p.hist_c[it] = c; p.hist_a[it] = (unsigned char)accept; }
-        if (stop) { done = true; return true; }
-        if (accept) {
-            kap = jacc < C::KAPN ? sKap[jacc] : (T)kappa_tab[jacc];
-            ++jacc;
-        } else {
-            kap = (T)0; jacc = 0;
+        if (lane == 0) {
+            const double c = p.rho * sum, c_last = red[32];
+            const bool stop = p.tol > 0.0 && c < p.tol;
+            const bool accept = !stop && c <= p.eta * c_last;
+            *reinterpret_cast<volatile int *>(sDec) = stop ? 2 : (accept ? 0 : 1);
+            if (cta == 0 && p.hist_c && it < p.hist_cap) { p.hist_c[it] = c; p.hist_a[it] = (unsigned char)accept; }
+            red[33] = c_last; red[32] = c; sCtl[2] = it + 1; sCtl[3] = stop;
+            if (accept) ++sCtl[0];
+            else if (!stop) { sCtl[0] = 0; ++sCtl[1]; }
         }
-        return false;
     };
 
-    bool in_b = false;                           // which of (sa, sb) holds the current iterate
-    for (int it = 0; it < iters; it += 2) {
-        if (iteration(sa, sb, it, 0)) { in_b = true; break; }
-        in_b = true;
-        if (it + 1 >= iters) break;
-        if (iteration(sb, sa, it + 1, 1)) { in_b = false; break; }
-        in_b = false;
+    // Barriers: bar_all = every warp of the CTA; bar_cmp = the compute warps only (named barrier 1), so that the communication
+    // warp can sit in the exchange while the compute warps hand phase A to phase B.
+    auto bar_all = [&]() { __syncthreads(); };
+    auto bar_cmp = [&]() { if (!comm) asm volatile("bar.sync 1, %0;" ::"r"(ncw * 32) : "memory"); };
+
+    // One iteration of Alg. 1 on (cur, prv) = iterates i, i-1; par = it & 1.  On entry phase A of this iteration has run; with
+    // `pending` the decision of iteration it-1 is still open: the hats were formed with the momentum of an ACCEPTED step
+    // (speculation) and the communication warp is summing / exchanging the partials of c and deciding
+    // while the compute warps fetch the ghosts and run phases A, B, C; everybody resolves it before phase D, the first point
+    // that overwrites an iterate.  A restart repeats A, B, C with kappa = 0.  Returns 0: go on, 1: iteration it-1 stopped
+    // (iterate = cur), 2: this iteration stopped (iterate = prv).
+    // Prediction: restart after two restarts in a row, else accept -- the accelerated phase restarts once every few steps
+    // (C4: every 7th), a slowly converging tail restarts EVERY step (C2 / C3 after ~300 iterations: c falls by less than
+    // eta per step), and both are then predicted right.  jacc counts RESOLVED accepted steps.
+    bool pending = false, pred_restart = false;
+    unsigned hist = 0;                                         // resolved decisions, newest in bit 0 (1 = restart)
+    auto kappa_of = [&](int j) -> T { return j < C::KAPN ? sKap[j] : (T)kappa_tab[j]; };
+    auto iteration = [&](OState<T> (&cur)[SPG], OState<T> (&prv)[SPG], const int it, const int par) -> int {
+        bar_cmp();                                             // w, vhat - betahat of the neighbour stages
+        phaseBC(par);
+        if (pending) {
+            bar_all();                                         // the communication warp has published the decision of iteration it-1
+            const int dec = *reinterpret_cast<volatile int *>(sDec);
+            if (dec == 2) return 1;
+            hist = (hist << 1) | (unsigned)(dec == 1);
+            bool redo = false;
+            if (dec == 0) {
+                const T kacc = kappa_of(jacc);
+                ++jacc;
+                if (pred_restart) { kap = kacc; phaseA(cur, prv); redo = true; }
+            } else {
+                jacc = 0;
+                if (!pred_restart) { kap = (T)0; phaseA_restart(cur); redo = true; }
+            }
+            if (redo) {                                        // mis-predicted: A, B, C again with the right momentum
+                bar_cmp();
+                phaseBC(par);
+                bar_cmp();
+            }
+            pending = false;
+        } else {
+            bar_cmp();                                         // xbar, Delta u of the neighbour stages
+        }
+        phaseD(prv, it, par);
+        bar_all();                                             // every lane's partial of c is in shared memory
+        decide(it);                                            // communication warp; the others go on
+        ghosts(prv, it, par);
+        if (!spec || it + 1 >= iters) {                        // wait for the decision
+            bar_all();
+            const int dec = *reinterpret_cast<volatile int *>(sDec);
+            if (dec == 2) return 2;
+            hist = (hist << 1) | (unsigned)(dec == 1);
+            if (dec == 0) { kap = kappa_of(jacc); ++jacc; }
+            else { kap = (T)0; jacc = 0; }
+            if (it + 1 < iters) phaseA(prv, cur);              // the new iterate sits in prv's registers
+        } else {
+            pred_restart = (hist & 3u) == 3u;
+            pending = true;
+            if (pred_restart) { kap = (T)0; phaseA_restart(prv); }
+            else { kap = kappa_of(jacc); phaseA(prv, cur); }
+        }
+        return 0;
+    };
+
+    int fin_b = 0, last_par = 1;                 // which of (sa, sb) holds the returned iterate; parity of the iteration that made it
+    if (iters > 0) phaseA(sa, sb);               // kappa = 0: hats = iterates (Alg. 1 input)
+    for (int it = 0;; it += 2) {
+        if (it >= iters) { fin_b = 0; last_par = 1; break; }
+        int r = iteration(sa, sb, it, 0);
+        if (r == 1) { fin_b = 0; last_par = 1; break; }
+        if (r == 2 || it + 1 >= iters) { fin_b = 1; last_par = 0; break; }
+        r = iteration(sb, sa, it + 1, 1);
+        if (r == 1) { fin_b = 1; last_par = 0; break; }
+        if (r == 2 || it + 2 >= iters) { fin_b = 0; last_par = 1; break; }
     }
-    // ---- results: iterate -> S[i_cur], xbar and Delta u of the last iteration, control block ----
+    // ---- results: iterate -> S[i_cur], xbar and Delta u of the iteration that made it, control block ----
 #pragma unroll
     for (int s = 0; s < SPG; ++s) {
-        if (in_b) sa[s] = sb[s];                 // register moves; a reference select would force local memory
+        if (fin_b) sa[s] = sb[s];                // register moves; a reference select would force local memory
         if (!(real[s] && rowok)) continue;
         const int k = k0 - 1 + s * ngroups + g;
         T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(0, k);
         rec[p.oZ() + gi] = sa[s].z; rec[p.oV() + gi] = sa[s].v; rec[p.oTH() + gi] = sa[s].th;
         rec[p.oBE() + gi] = sa[s].be; rec[p.oLA() + gi] = sa[s].la;
-        p.X[(size_t)k * nb + gi] = blkp[s][OX + li];
+        p.X[(size_t)k * nb + gi] = blkp[s][OX + last_par * LPS + li];
         if (li >= NX) {
-            p.DU[(size_t)k * nu + (gi - nx)] = blkp[s][ODU + li - NX];
+            p.DU[(size_t)k * nu + (gi - nx)] = blkp[s][ODU + last_par * NUP + li - NX];
             if (DU) { rec[p.oD() + (gi - nx)] = sa[s].d; rec[p.oDE() + (gi - nx)] = sa[s].de; }
         }
     }
-    if (cta == 0 && tid == 0) {
+    if (cta == 0 && comm && lane == 0) {
         InstCtl c = p.ctl[0];
-        const int last = (it_done - 1) & 1;
-        c.alpha = alpha_tab[jacc]; c.c_last = it_done ? red[32 + last] : p.c0;
-        c.c_prev = done ? red[32 + (last ^ 1)] : c.c_last;
-        c.kappa = (double)kap;
-        c.done = done ? 1 : 0; c.iters = it_done; c.restarts = restarts;
+        const int r_jacc = sCtl[0], r_done = sCtl[3];
+        c.alpha = alpha_tab[r_jacc]; c.c_last = red[32];
+        c.c_prev = r_done ? red[33] : red[32];
+        c.kappa = r_jacc > 0 ? (double)(T)kappa_tab[r_jacc - 1] : 0.0;          // momentum of the last hats formed
+        c.done = r_done ? 1 : 0; c.iters = sCtl[2]; c.restarts = sCtl[1];
         p.ctl[0] = c;
     }
     if (CL) cluster_sync_all();                  // no CTA leaves while a peer could still address its shared memory
@@ -599,7 +703,7 @@ bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
     while (spg <= spg_max && ((slots + spg - 1) / spg + gpw - 1) / gpw > 31) ++spg;
     if (spg > spg_max) { if (why) *why = "horizon too long for the register-resident iterates of the COOP engine"; return false; }
     const int ncw = ((slots + spg - 1) / spg + gpw - 1) / gpw;
-    const size_t smem = C::smem_bytes(slots);
+    const size_t smem = C::smem_bytes(slots, (ncw + 1) * 32);
     if (smem > h->smem_optin) { if (why) *why = "stage matrices of a CTA's range do not fit in shared memory"; return false; }
     pl->grid = grid; pl->spg = spg; pl->threads = (ncw + 1) * 32; pl->slots = slots; pl->smem = smem; pl->cluster = cluster;
     return true;
@@ -611,6 +715,7 @@ int launch_coop(pimpc_s *h, int iters, double tol, const CoopPlan &pl)
     using C = OCfg<T, NX, NU>;
     typedef typename Tagged<double>::W PW;
     typedef typename Tagged<T>::W HW;
+    int spec = h->tune.lookahead >= 0 ? 1 : 0;                 // speculate the accept / restart decision unless opts.tune.lookahead = -1
     if (pl.cluster > 0) {
         // one thread-block cluster: co-scheduled by the hardware, exchange through distributed shared memory
         auto kc = h->has_du ? k_coop<T, NX, NU, SPG, MAXT, true, true> : k_coop<T, NX, NU, SPG, MAXT, false, true>;
@@ -626,7 +731,7 @@ int launch_coop(pimpc_s *h, int iters, double tol, const CoopPlan &pl)
         if (cudaOccupancyMaxActiveClusters(&ncl, kc, &cfg) == cudaSuccess && ncl >= 1) {
             Prob<T> pc = make_prob<T>(h, tol);
             const double *atc = h->alpha_tab, *ktc = h->kappa_tab;
-            PIMPC_CUDA_TRY(h, cudaLaunchKernelEx(&cfg, kc, pc, atc, ktc, iters, (PW *)nullptr, (HW *)nullptr));
+            PIMPC_CUDA_TRY(h, cudaLaunchKernelEx(&cfg, kc, pc, atc, ktc, iters, (PW *)nullptr, (HW *)nullptr, spec));
             h->info.grid = pl.grid; h->info.block = pl.threads; h->info.smem_bytes = pl.smem;
             return 1;
         }
@@ -645,7 +750,7 @@ int launch_coop(pimpc_s *h, int iters, double tol, const CoopPlan &pl)
     PW *part = (PW *)h->coop_buf;
     HW *halo = (HW *)((unsigned char *)h->coop_buf + pbytes);
     const double *at = h->alpha_tab, *kt = h->kappa_tab;
-    void *args[] = {(void *)&p, (void *)&at, (void *)&kt, (void *)&iters, (void *)&part, (void *)&halo};
+    void *args[] = {(void *)&p, (void *)&at, (void *)&kt, (void *)&iters, (void *)&part, (void *)&halo, (void *)&spec};
     PIMPC_CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)kern, dim3(pl.grid), dim3(pl.threads), args, pl.smem, h->stream));
     h->info.grid = pl.grid; h->info.block = pl.threads; h->info.smem_bytes = pl.smem;
     return 1;

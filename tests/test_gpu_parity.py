@@ -179,9 +179,11 @@ def test_stream_engine_early_stop_and_warm_start(oracle, pimpc, grid):
 
 
 # ---- COOP engine (batch 1, horizon spread over the SMs, tagged-word exchange instead of grid barriers) ------
-def _coop(grid=0, spg=0, cluster=None):
-    """cluster None: automatic (one cluster for short horizons); 0: exchange through L2 (the long-horizon path); n: cluster of n."""
-    return _tune(grid=grid, stages_per_group=spg, cluster=(0 if cluster is None else (-1 if cluster == 0 else cluster)))
+def _coop(grid=0, spg=0, cluster=None, lookahead=0):
+    """cluster None: automatic (one cluster for short horizons); 0: exchange through L2 (the long-horizon path); n: cluster of n.
+    lookahead -1: every thread waits for the accept / restart decision instead of predicting it."""
+    return _tune(grid=grid, stages_per_group=spg, cluster=(0 if cluster is None else (-1 if cluster == 0 else cluster)),
+                 lookahead=lookahead)
 
 
 @pytest.mark.parametrize("cluster", [None, 0, 8])
@@ -194,6 +196,8 @@ def test_coop_engine_all_options(oracle, pimpc, shape, grid, dtype, cluster):
     nx, nu, N = shape
     if N > 100 and grid in (1, 2):
         grid += 4                         # 150 stages of (12, 4) do not fit one or two CTAs' shared memory: 5, 6 CTAs
+    if (nx, N, grid, dtype) == (12, 41, 1, "f64"):
+        grid = 3                          # 41 fp64 stages of (12, 4) no longer fit ONE CTA (parity copies of xbar, lane partials of c)
     p = wl.random_ltv(nx, nu, N, 1, seed=nx * 10 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
                       qbar=True, bounds=0.8, du_bound=0.5)
     g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="coop", iters=120, tol=0.0, opts=_coop(grid, cluster=cluster))
@@ -207,6 +211,28 @@ def test_coop_engine_two_stages_per_group_fp32(oracle, pimpc, grid, cluster):
     p = wl.random_ltv(12, 4, 100, 1, seed=5, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
     g, worst, nrep = parity.check(oracle, pimpc, p, "f32", engine="coop", iters=150, tol=0.0, opts=_coop(grid, 2, cluster))
     assert g["info"]["engine"] == pimpc.ENGINE_COOP
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("cluster", [None, 0])
+@pytest.mark.parametrize("shape,grid", [((12, 4, 41), 0), ((12, 4, 150), 7), ((4, 2, 23), 2)])
+def test_coop_decision_predicted_or_waited_for(oracle, pimpc, shape, grid, cluster, dtype):
+    """by default the compute warps PREDICT the accept / restart decision and run phases A-C of the next
+    iteration while the partial sums of c travel (a wrong prediction repeats them); tune.lookahead = -1 makes them wait.
+    Both orders must give the oracle's iterates and decision sequence; 400 iterations reach the all-restart tail, so that
+    accept-predicted-restart, restart-predicted-accept and the right predictions all occur."""
+    nx, nu, N = shape
+    p = wl.random_ltv(nx, nu, N, 1, seed=nx * 7 + N, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
+    res = {}
+    for la in (0, -1):
+        g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="coop", iters=400, tol=0.0,
+                                      opts=_coop(grid, cluster=cluster, lookahead=la))
+        assert g["info"]["engine"] == pimpc.ENGINE_COOP
+        res[la] = g
+    for name in ("Z", "V", "TH", "BE", "LA", "X", "DU"):
+        assert np.array_equal(res[0][name], res[-1][name]), name       # same arithmetic in both orders: bit-identical
+    assert np.array_equal(res[0]["acc_hist"], res[-1]["acc_hist"])
+    assert 0 < int(res[0]["res"]["restarts"][0]) < 400
 
 
 @pytest.mark.parametrize("cluster", [None, 0])
