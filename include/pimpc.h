@@ -118,6 +118,17 @@ typedef struct {
     double smem_gbs;      /* conflict-free 16-byte shared-memory loads, all SMs                         */
     int sm_count;
     int pad_;
+    /* Latencies of one dependent instruction (SM cycles, one warp alone on an SM, clock64 around a chain): what an in-order
+     * warp pays per step of a dependency chain -- the register-resident kernels run 3-4 warps per scheduler in lock-step
+     * phases, so these, not the pipe rates above, set the length of a phase. */
+    double lat_ffma2_cycles;  /* fma.rn.f32x2 -> fma.rn.f32x2                                               */
+    double lat_dadd_cycles;   /* add.f64 -> add.f64                                                         */
+    double lat_shfl_cycles;   /* shfl.sync.bfly -> shfl.sync.bfly                                           */
+    double lat_lds_cycles;    /* ld.shared (pointer chase)                                                  */
+    /* Shared-memory pipe cycles per warp-wide 16-byte load when groups of 8 lanes read the same 16 bytes (the broadcast
+     * vector loads of the RESIDENT engine), 16 warps per SM, addresses moving every iteration; a load with 32 distinct
+     * addresses takes 4 (smem_gbs above). */
+    double lds128_bcast_cycles;
 } pimpc_peaks;
 
 const char *pimpc_version(void);

@@ -57,7 +57,9 @@ class pimpc_info(ctypes.Structure):
 
 class pimpc_peaks(ctypes.Structure):
     _fields_ = [("ffma_tflops", ctypes.c_double), ("ffma2_tflops", ctypes.c_double), ("dfma_tflops", ctypes.c_double),
-                ("smem_gbs", ctypes.c_double), ("sm_count", ctypes.c_int), ("pad_", ctypes.c_int)]
+                ("smem_gbs", ctypes.c_double), ("sm_count", ctypes.c_int), ("pad_", ctypes.c_int),
+                ("lat_ffma2_cycles", ctypes.c_double), ("lat_dadd_cycles", ctypes.c_double), ("lat_shfl_cycles", ctypes.c_double),
+                ("lat_lds_cycles", ctypes.c_double), ("lds128_bcast_cycles", ctypes.c_double)]
 
 
 RESULT_DTYPE = np.dtype([("c", "f8"), ("alpha", "f8"), ("r_prim2", "f8"), ("r_dual2", "f8"), ("iters", "i4"),
