@@ -209,9 +209,11 @@ __global__ void __launch_bounds__(128) k_setup_small(Prob<T> p, const int *__res
     for (int j = 0; j < LPS; ++j) buf[li * TS + j] = S[j];
     __syncwarp();
     if (act && rowok) {
-        T *Hk = p.H + (size_t)sidx * NB * NB + (size_t)li * NB;
+        // row i by the lanes of the group (coalesced: a lane-per-row store touched 32 sectors per instruction, and the LSU pipe
+        // was 90 % busy): H[i][li] = (S_i[li] + S_li[i]) / 2, exactly symmetric
+        T *Hs = p.H + (size_t)sidx * NB * NB + li;
 #pragma unroll
-        for (int j = 0; j < NB; ++j) Hk[j] = (T)(0.5 * (S[j] + buf[j * TS + li]));      // exactly symmetric
+        for (int i = 0; i < NB; ++i) Hs[i * NB] = (T)(0.5 * (buf[i * TS + li] + S[i]));
     }
     __syncwarp();
 
@@ -239,9 +241,9 @@ __global__ void __launch_bounds__(128) k_setup_small(Prob<T> p, const int *__res
     }
     __syncwarp();
     if (act && li < NU) {
-        T *Mk = p.M + (size_t)sidx * NU * NU + (size_t)li * NU;
+        T *Ms = p.M + (size_t)sidx * NU * NU + li;
 #pragma unroll
-        for (int j = 0; j < MW; ++j) Mk[j] = (T)(0.5 * (Mr[j] + buf[j * TS + li]));
+        for (int i = 0; i < MW; ++i) Ms[i * NU] = (T)(0.5 * (buf[i * TS + li] + Mr[i]));
     }
     if (!finite) atomicOr(p.err, PIMPC_DEVERR_NONFINITE);
     else if (!ok) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
