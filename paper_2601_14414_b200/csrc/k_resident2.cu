@@ -8,7 +8,7 @@
 //
 // Per-solve prologue (registers of the row owner, read from HBM once per solve):
 //   Hrow  row of H_k
-//   G     row of G_k = rho H_k [A_{k+1} B_{k+1}]^T  (nb x nx), formed in double   -- step 1 re-associated:
+//   G     row of G_k = rho H_k [A_{k+1} B_{k+1}]^T  (nb x nx)                     -- step 1 re-associated:
 //           xbar_{k+1} = H_k h_k,  h_k = qbar + rho (zhat - thetahat) + rho Abar_{k+1}^T w_{k+1}   (R2)
 //                      = H_k (t_k + rho [0; w_u]) + G_k w_x,   t_k = qbar + rho (zhat - thetahat),
 //         so the transposed product with Abar_{k+1} (columns in shared memory, a dependent second mat-vec in round 1)
@@ -69,6 +69,17 @@ __device__ __forceinline__ void ld4p(const double *p, double2 &a, double2 &b)
 {
     a = *reinterpret_cast<const double2 *>(p); b = *reinterpret_cast<const double2 *>(p + 2);
 }
+// 4 consecutive elements of global memory (16-byte aligned in fp32, 32-byte in fp64)
+__device__ __forceinline__ void ldg4(const float *p, float (&o)[4])
+{
+    const float4 v = __ldg(reinterpret_cast<const float4 *>(p));
+    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void ldg4(const double *p, double (&o)[4])
+{
+    const double2 a = __ldg(reinterpret_cast<const double2 *>(p)), b = __ldg(reinterpret_cast<const double2 *>(p + 2));
+    o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
+}
 __device__ __forceinline__ float2 ldp(const float *p) { return *reinterpret_cast<const float2 *>(p); }
 __device__ __forceinline__ double2 ldp(const double *p) { return *reinterpret_cast<const double2 *>(p); }
 __device__ __forceinline__ void stp(float *p, float2 v) { *reinterpret_cast<float2 *>(p) = v; }
@@ -128,7 +139,6 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     using P = typename Pr<T>::t;
     constexpr int NBP = C::NBP, LPS = C::LPS, SPW = C::SPW, SS = C::SS;
     constexpr int OW = C::OW, OT = C::OT, ORR = C::ORR, OX = C::OX, ODU = C::ODU, OE = C::OE, OG = C::OG, ROWP = C::ROWP;
-    constexpr int NG = GS ? 1 : NXP;                          // register copy of G only when it is not in shared memory
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nmain = (blockDim.x >> 5) - 1;                  // warps 0..nmain-1 own stages, warp nmain is the reducer
@@ -163,10 +173,47 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     int pit = 0;
 #endif
     for (int b = blockIdx.x; b < p.batch; b += gridDim.x) {
+        // ---- [A_k B_k] of every stage of the instance -> the stage's slot (the area that later holds G_k), padded, by ONE
+        // coalesced cooperative load of the whole CTA: the per-solve prologue then forms U, J_k and G_k from shared memory
+        // (per-lane rolled loops over global memory made the prologue 0.67 ms of C4's 7.15 ms kernel)
+        for (int i0 = tid; i0 < NS * NXP * ROWP; i0 += 4 * blockDim.x) {
+            T v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {                      // four independent loads in flight per thread
+                const int i = i0 + u * blockDim.x;
+                const int ks = i / (NXP * ROWP), q = i - ks * (NXP * ROWP), r = q / ROWP, c = q - r * ROWP;
+                v[u] = (T)0;
+                if (ks < N && r < nx && c < NBP) {
+                    const size_t st = (size_t)b * N + ks;
+                    if (c < NXP) { if (c < nx) v[u] = p.A[st * nx * nx + r * nx + c]; }
+                    else if (c - NXP < nu) v[u] = p.B[st * nx * nu + r * nu + (c - NXP)];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int i = i0 + u * blockDim.x;
+                if (i < NS * NXP * ROWP) { const int ks = i / (NXP * ROWP); sBlk[(size_t)(ks + 1) * SS + OG + (i - ks * (NXP * ROWP))] = v[u]; }
+            }
+        }
+        __syncthreads();
         if (warp == nmain) {
             // ---- the reducer warp: step 4's sum and steps 5-7 for the whole CTA.  It follows the barrier
             // sequence of the stage warps: per iteration bar1 (phase A published | partial sums of the previous iteration
             // complete), bar2 (phase B done | decision published), two more after a restart.
+            // the next instance of this CTA: its stage data and iterates -> L2 while this one iterates (the reducer warp has the
+            // time), so that the next prologue pays L2 instead of HBM latencies
+            if (b + (int)gridDim.x < p.batch) {
+                const size_t bn = (size_t)b + gridDim.x;
+                auto pf = [&](const void *base, size_t bytes) {
+                    for (size_t o = (size_t)lane * 128; o < bytes; o += 32 * 128)
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(base) + o));
+                };
+                pf(p.A + bn * N * nx * nx, (size_t)N * nx * nx * sizeof(T));
+                pf(p.B + bn * N * nx * nu, (size_t)N * nx * nu * sizeof(T));
+                pf(p.H + bn * N * nb * nb, (size_t)N * nb * nb * sizeof(T));
+                pf(p.M + bn * N * nu * nu, (size_t)N * nu * nu * sizeof(T));
+                pf(p.S + (size_t)p.ctl[bn].i_cur * p.buf_stride + p.st((int)bn, 0), (size_t)N * p.rec * sizeof(T));
+            }
             double c_last = p.c0, c_prev = p.c0, thr = p.eta * p.c0;   // thr = eta c^{i}: ready before c^{i+1} arrives
             int jacc = 0, nrest = 0, n_it = 0;
             bool done = false;
@@ -229,44 +276,65 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         const int i_cur = p.ctl[b].i_cur;
         const size_t sk = (size_t)b * N + (stage_ok ? k : 0);
         const bool inner = stage_ok && k < N - 1;
+        const bool native = nx == NXP && nu == NUP;            // no pad rows / columns: row-major H_k rows are NBP contiguous elements
         // ---- stage matrices -> registers (once per solve) ----------------------------------------------------------
-        T Hrow[2][NBP], G[2][NG], U[2][NBP];
+        T Hrow[2][NBP], G[2][NXP], U[2][NBP];
         R2State<P> sa, sb;
         {
-            // J_k = M_k Bbar_k^T: its nu x nx block M_k B_k^T is formed by the whole lane group (rolled loops,
-            // double accumulation) in the scratch that later holds G_k, then picked up by the u rows
-            if (stage_ok) {
-                const T *Bk = p.B + sk * nx * nu, *Mk = p.M + sk * nu * nu;
-#pragma unroll 1
-                for (int e = li; e < NUP * NXP; e += LPS) {
-                    const int iu = e / NXP, j = e - iu * NXP;
-                    double s = 0.0;
-                    if (iu < nu && j < nx)
-                        for (int c = 0; c < nu; ++c) s += (double)Mk[iu * nu + c] * (double)Bk[j * nu + c];
-                    blk[OG + e] = (T)s;
-                }
-            }
-            __syncwarp();
+            const T *const ab = blk + OG, *const ab1 = blk + SS + OG;          // [A_k B_k], [A_{k+1} B_{k+1}] as [NXP][ROWP]
             T st_[7][2];
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
                 const int gi = gidx(i0 + r);
                 const bool ok = stage_ok && gi >= 0;
-                const bool okx = ok && i0 < NXP, oku = ok && i0 >= NXP;
+                const bool oku = ok && i0 >= NXP;
                 const T *Hk = p.H + sk * nb * nb + (size_t)(ok ? gi : 0) * nb;
+                if (native) {                                          // unpadded shape: 16-byte loads of the row (a scalar load per
+                                                                       // element touched 32 sectors per instruction, 16 times per row)
 #pragma unroll
-                for (int j = 0; j < NBP; ++j) { const int gj = gidx(j); Hrow[r][j] = (ok && gj >= 0) ? Hk[gj] : (T)0; }
-                const T *Ak = p.A + sk * nx * nx, *Bk = p.B + sk * nx * nu, *Mk = p.M + sk * nu * nu;
+                    for (int j = 0; j < NBP; j += 4) {
+                        T h4[4] = {(T)0, (T)0, (T)0, (T)0};
+                        if (ok) ldg4(Hk + j, h4);
+                        Hrow[r][j] = h4[0]; Hrow[r][j + 1] = h4[1]; Hrow[r][j + 2] = h4[2]; Hrow[r][j + 3] = h4[3];
+                    }
+                } else {
 #pragma unroll
-                for (int j = 0; j < NBP; ++j) {
-                    const int gj = gidx(j);
-                    T v = (T)0;
-                    if (okx && gj >= 0) v = j < NXP ? Ak[gi * nx + gj] : Bk[gi * nu + (gj - nx)];          // row of [A_k B_k]
-                    else if (oku && gj >= 0) v = j >= NXP ? Mk[(size_t)(gi - nx) * nu + (gj - nx)]        // row of M_k
-                                                         : blk[OG + (i0 + r - NXP) * NXP + j];                // row of M_k B_k^T (staged below)
-                    U[r][j] = v;
+                    for (int j = 0; j < NBP; ++j) { const int gj = gidx(j); Hrow[r][j] = (ok && gj >= 0) ? Hk[gj] : (T)0; }
                 }
-                own[OE + r] = (okx && has_e) ? p.e[sk * nx + gi] : (T)0;
+                if (i0 < NXP) {                                        // x rows: row of [A_k B_k] (pad rows and pad stages: zeros)
+#pragma unroll
+                    for (int j = 0; j < NBP; ++j) U[r][j] = ab[(i0 + r) * ROWP + j];
+                } else {
+                    // u rows: row of J_k = M_k Bbar_k^T = [M_k B_k^T | M_k], the paper's cached J_k
+                    T mrow[NUP];
+#pragma unroll
+                    for (int c = 0; c < NUP; ++c) mrow[c] = (oku && c < nu) ? p.M[sk * nu * nu + (size_t)(gi - nx) * nu + c] : (T)0;
+#pragma unroll
+                    for (int j = 0; j < NXP; ++j) {
+                        T acc = (T)0;
+#pragma unroll
+                        for (int c = 0; c < NUP; ++c) acc = fma(mrow[c], ab[j * ROWP + NXP + c], acc);
+                        U[r][j] = acc;
+                    }
+#pragma unroll
+                    for (int c = 0; c < NUP; ++c) U[r][NXP + c] = mrow[c];
+                }
+                own[OE + r] = (ok && i0 < NXP && has_e) ? p.e[sk * nx + gi] : (T)0;
+                // G_k row = rho * Hrow . [A_{k+1} B_{k+1}]^T in the arithmetic of the handle (two accumulators per entry; in fp32 a
+                // 16-term product sum is good to ~4e-7 relative, two orders below the iterate error the fp32 path carries anyway)
+#pragma unroll
+                for (int j = 0; j < NXP; ++j) {
+                    T a0 = (T)0, a1 = (T)0;
+                    if (inner) {
+#pragma unroll
+                        for (int c4 = 0; c4 < NBP; c4 += 4) {
+                            const T *q = ab1 + j * ROWP + c4;
+                            a0 = fma(Hrow[r][c4], q[0], a0); a1 = fma(Hrow[r][c4 + 1], q[1], a1);
+                            a0 = fma(Hrow[r][c4 + 2], q[2], a0); a1 = fma(Hrow[r][c4 + 3], q[3], a1);
+                        }
+                    }
+                    G[r][j] = rho * (a0 + a1);
+                }
                 // ---- iterate of the previous solve / cold start (hats = iterates: prev = cur) ----
                 const T *rec = p.S + (size_t)i_cur * p.buf_stride + p.st(b, stage_ok ? k : 0);
                 st_[0][r] = ok ? rec[p.oZ() + gi] : (T)0;
@@ -276,34 +344,6 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 st_[4][r] = ok ? rec[p.oLA() + gi] : (T)0;
                 st_[5][r] = (oku && DU) ? rec[p.oD() + (gi - nx)] : (T)0;
                 st_[6][r] = (oku && DU) ? rec[p.oDE() + (gi - nx)] : (T)0;
-            }
-            __syncwarp();                                      // the scratch is reused
-            // G_k rows = rho * Hrow . [A_{k+1} B_{k+1}]^T, accumulated in double (the factors are the rounded inputs); a
-            // rolled loop over the nx rows of [A_{k+1} B_{k+1}], every element loaded once for both rows of the lane
-            {
-                const T *A1 = p.A + (sk + (inner ? 1 : 0)) * nx * nx, *B1 = p.B + (sk + (inner ? 1 : 0)) * nx * nu;
-#pragma unroll 1
-                for (int j = 0; j < NXP; ++j) {
-                    double s0 = 0.0, s1 = 0.0;
-                    if (inner && j < nx) {
-#pragma unroll
-                        for (int c = 0; c < NBP; ++c) {
-                            const int gc = gidx(c);
-                            if (gc >= 0) {
-                                const double a = (double)(c < NXP ? A1[j * nx + gc] : B1[j * nu + (gc - nx)]);
-                                s0 += (double)Hrow[0][c] * a; s1 += (double)Hrow[1][c] * a;
-                            }
-                        }
-                    }
-                    blk[OG + ((0 * (NXP / 2) + j / 2) * LPS + li) * 2 + (j & 1)] = (T)(p.rho * s0);
-                    blk[OG + ((1 * (NXP / 2) + j / 2) * LPS + li) * 2 + (j & 1)] = (T)(p.rho * s1);
-                }
-                if (!GS) {
-#pragma unroll
-                    for (int r = 0; r < 2; ++r)
-#pragma unroll
-                        for (int j = 0; j < NXP; ++j) G[r][j % NG] = blk[OG + ((r * (NXP / 2) + j / 2) * LPS + li) * 2 + (j & 1)];
-                }
             }
             sa.z = mk2(st_[0][0], st_[0][1]); sa.v = mk2(st_[1][0], st_[1][1]); sa.th = mk2(st_[2][0], st_[2][1]);
             sa.be = mk2(st_[3][0], st_[3][1]); sa.la = mk2(st_[4][0], st_[4][1]);
@@ -398,7 +438,7 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
 #pragma unroll
                 for (int c2 = 0; c2 < NXP / 2; ++c2)
 #pragma unroll
-                    for (int r = 0; r < 2; ++r) xa[r] = fma2(mk2(G[r][(2 * c2) % NG], G[r][(2 * c2 + 1) % NG]), wv[c2], xa[r]);
+                    for (int r = 0; r < 2; ++r) xa[r] = fma2(mk2(G[r][2 * c2], G[r][2 * c2 + 1]), wv[c2], xa[r]);
             }
             xs = mk2(xa[0].x + xa[0].y, xa[1].x + xa[1].y);
             du = mk2(da[0].x + da[0].y, da[1].x + da[1].y);                      // meaningful on the u rows only
@@ -527,7 +567,13 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             }
         };
 
-        __syncthreads();
+        __syncthreads();                                       // every stage has read its neighbour's [A B]; slot 0 and the boxes are in place
+        if (GS) {                                              // G_k -> the slot (lane-major 8-byte pieces), over the staged [A_k B_k]
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                for (int c2 = 0; c2 < NXP / 2; ++c2) stp(blk + OG + ((r * (NXP / 2) + c2) * LPS + li) * 2, mk2(G[r][2 * c2], G[r][2 * c2 + 1]));
+        }
 #ifdef R2_PROF
         pit = 0; R2P(5); pit = 1;
 #endif
