@@ -303,9 +303,10 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
     int jacc = 0;                                // accepted steps in a row, a pending (speculated) one counted as accepted
     unsigned long long xold[2][3] = {{0ull, 0ull, 0ull}, {0ull, 0ull, 0ull}};     // this CTA's limbs still inside the two parity slots
     // the accept / restart state of Alg. 1 lives in shared memory (lane 0 of the communication warp reads and writes it):
-    // red[32] = c of the last iteration, red[33] = c of the one before; sCtl = {accepted steps in a row, restarts, iterations, done}
+    // red[32] = c of the last iteration, red[33] = c of the one before, red[38] = eta * red[32], red[39] = c of the decision whose
+    // bookkeeping is pending; sCtl = {accepted steps in a row, restarts, iterations, done}
     int *sCtl = reinterpret_cast<int *>(red + 36);
-    if (tid == 0) { red[32] = p.c0; red[33] = p.c0; sCtl[0] = sCtl[1] = sCtl[2] = sCtl[3] = 0; }
+    if (tid == 0) { red[32] = p.c0; red[33] = p.c0; red[38] = p.eta * p.c0; sCtl[0] = sCtl[1] = sCtl[2] = sCtl[3] = 0; }
     const int slots_max = (N + G - 1) / G + 2;
     T *sAcc = sBlk + (size_t)slots_max * SS;     // [2][blockDim.x] per-lane partial sums of c by parity of the iteration
     int *sDec = reinterpret_cast<int *>(red + 34);   // decision of the communication warp: 0 accept, 1 restart, 2 stop
@@ -519,9 +520,10 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         // fixed order: this lane's column over the compute warps (loads in flight together, a balanced tree in T), the butterfly
         // over the lanes, then double
         const T *a = sAcc + par * blockDim.x + lane;
+        const double thr = red[38];                            // eta c^{i}: fetched before the sums
         T sT = (T)0;
-#pragma unroll
-        for (int j0 = 0; j0 < 32; j0 += 8) {                   // eight warps at a time (register budget of the 1024-thread variants)
+#pragma unroll 1
+        for (int j0 = 0; j0 < ncw; j0 += 8) {                  // eight warps at a time (short ranges: one batch)
             T v[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) v[j] = j0 + j < ncw ? a[(j0 + j) * 32] : (T)0;
@@ -540,7 +542,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             if (lane < G) while (!TD::ld_sm(xPart + par * C::CLMAX + lane, tag, val)) {}
             sum = val;
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            for (int o = 8; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);       // a cluster has at most 16 CTAs
         } else {
             // exact fixed-point atomic sum (see to_limbs): parity slot, three adjacent words, never reset
             unsigned long long *acc = reinterpret_cast<unsigned long long *>(part) + (size_t)par * 32;
@@ -561,16 +563,23 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             }
             sum = __shfl_sync(0xffffffffu, sum, 0);
         }
-        if (lane == 0) {
-            const double c = p.rho * sum, c_last = red[32];
+        if (lane == 0) {                                       // the decision word first: the compute warps wait for it
+            const double c = p.rho * sum;
             const bool stop = p.tol > 0.0 && c < p.tol;
-            const bool accept = !stop && c <= p.eta * c_last;
+            const bool accept = !stop && c <= thr;
             *reinterpret_cast<volatile int *>(sDec) = stop ? 2 : (accept ? 0 : 1);
-            if (cta == 0 && p.hist_c && it < p.hist_cap) { p.hist_c[it] = c; p.hist_a[it] = (unsigned char)accept; }
-            red[33] = c_last; red[32] = c; sCtl[2] = it + 1; sCtl[3] = stop;
-            if (accept) ++sCtl[0];
-            else if (!stop) { sCtl[0] = 0; ++sCtl[1]; }
+            red[39] = c;
         }
+    };
+    // the bookkeeping of that decision, off the critical path (after the barrier that hands the decision word over)
+    auto book = [&](const int it) {
+        if (!(comm && lane == 0)) return;
+        const double c = red[39];
+        const int dec = *reinterpret_cast<volatile int *>(sDec);
+        if (cta == 0 && p.hist_c && it < p.hist_cap) { p.hist_c[it] = c; p.hist_a[it] = (unsigned char)(dec == 0); }
+        red[33] = red[32]; red[32] = c; red[38] = p.eta * c; sCtl[2] = it + 1; sCtl[3] = dec == 2;
+        if (dec == 0) ++sCtl[0];
+        else if (dec == 1) { sCtl[0] = 0; ++sCtl[1]; }
     };
 
     // Barriers: bar_all = every warp of the CTA; bar_cmp = the compute warps only (named barrier 1), so that the communication
@@ -596,6 +605,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         if (pending) {
             bar_all();                                         // the communication warp has published the decision of iteration it-1
             const int dec = *reinterpret_cast<volatile int *>(sDec);
+            book(it - 1);
             if (dec == 2) return 1;
             hist = (hist << 1) | (unsigned)(dec == 1);
             bool redo = false;
@@ -623,6 +633,7 @@ k_coop(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         if (!spec || it + 1 >= iters) {                        // wait for the decision
             bar_all();
             const int dec = *reinterpret_cast<volatile int *>(sDec);
+            book(it);
             if (dec == 2) return 2;
             hist = (hist << 1) | (unsigned)(dec == 1);
             if (dec == 0) { kap = kappa_of(jacc); ++jacc; }
