@@ -215,7 +215,7 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 pf(p.S + (size_t)p.ctl[bn].i_cur * p.buf_stride + p.st((int)bn, 0), (size_t)N * p.rec * sizeof(T));
             }
             double c_last = p.c0, c_prev = p.c0, thr = p.eta * p.c0;   // thr = eta c^{i}: ready before c^{i+1} arrives
-            int jacc = 0, nrest = 0, n_it = 0;
+            int jacc = 0, nrest = 0, n_it = 0, lrun = 0;       // lrun: accepted steps before the last restart
             bool done = false;
             auto decide = [&](const int it) -> int {
                 // fixed order: this lane's column over the stage warps (all loads in flight at once, zeros beyond nmain, a
@@ -246,22 +246,35 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 }
                 c_prev = c_last; c_last = c; thr = p.eta * c; n_it = it + 1;
                 if (accept) ++jacc;
-                else if (!stop) { jacc = 0; ++nrest; }
+                else if (!stop) { lrun = jacc > 0 ? jacc : -1; jacc = 0; ++nrest; }      // -1: a restart right after a restart
                 done = stop;
                 return dec;
             };
             __syncthreads();
+            // Mirror of the stage warps' schedule (see `iteration`): a decision is either PREDICTED as "accept" and taken between
+            // barriers 1 and 2 of the next iteration (a restart then repeats A and B: two more barriers), or -- when the run of
+            // accepted steps has reached the length of the previous run, i.e. a restart is due -- WAITED for right after phase C.
             int it = 0;
+            bool resolved = true;                              // is the decision of iteration it-1 taken at the top of iteration it
 #pragma unroll 1
             for (; it < iters; ++it) {
                 __syncthreads();
                 int dec = 0;
-                if (it > 0) dec = decide(it - 1);
+                if (!resolved) dec = decide(it - 1);
                 __syncthreads();
-                if (dec == 2) break;
-                if (dec == 1) { __syncthreads(); __syncthreads(); }
+                if (!resolved) {
+                    if (dec == 2) break;
+                    if (dec == 1) { __syncthreads(); __syncthreads(); }
+                }
+                resolved = (lrun > 0 && jacc >= lrun) || (lrun < 0 && jacc == 0);
+                if (resolved) {
+                    __syncthreads();
+                    dec = decide(it);
+                    __syncthreads();
+                    if (dec == 2) break;
+                }
             }
-            if (!done && iters > 0) { __syncthreads(); decide(iters - 1); __syncthreads(); }
+            if (!done && !resolved) { __syncthreads(); decide(iters - 1); __syncthreads(); }
             if (lane == 0) {
                 InstCtl c = p.ctl[b];
                 c.alpha = alpha_tab[jacc]; c.c_last = c_last;
@@ -363,7 +376,8 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         }
 
         T kap = (T)0;                                          // momentum of the hats being formed
-        int jacc = 0;                                          // accepted steps in a row, the pending one counted as accepted
+        int jacc = 0, lrun = 0;                                // accepted steps in a row (a pending one counted as accepted), and before the last restart
+        bool pend = false;                                     // the decision of the previous iteration is still open
         P zh, vh, thh, beh, lah, dh, deh;                      // hats of the iteration in flight (A -> C)
         P xs, du;                                              // own rows of xbar_{k+1}, Delta u_k of the iteration in flight (B -> C)
         zh = vh = thh = beh = lah = dh = deh = xs = du = mk2((T)0, (T)0);
@@ -507,7 +521,7 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         // One iteration of Alg. 1 on (cur, prv) = iterates i, i-1; par = it & 1 (compile-time after unrolling by two).  On
         // entry phase A of this iteration has run (speculated momentum) and the decision of iteration it-1 is pending
         // (it > 0): the reducer warp takes it between the two barriers.  Returns true when iteration it-1 stopped (c < tol).
-        auto iteration = [&](R2State<P> &cur, R2State<P> &prv, const int it, const int par) -> bool {
+        auto iteration = [&](R2State<P> &cur, R2State<P> &prv, const int it, const int par) -> int {
 #ifdef R2_PROF
             if (blockIdx.x == 0 && lane == 0 && pit < 1024) g_r2prof[(pit * 16 + warp) * 8 + 4] = 0;
 #endif
@@ -518,10 +532,11 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             R2P(2);
             __syncthreads();
             R2P(3);
-            if (it > 0) {
+            if (pend) {
                 const int dec = *reinterpret_cast<volatile int *>(sDec);       // steps 5-7 of iteration it-1 (the reducer warp)
-                if (dec == 2) return true;
+                if (dec == 2) return 1;
                 if (dec == 1) {                                // restart: A and B again with kappa = 0
+                    lrun = jacc > 1 ? jacc - 1 : -1;           // (the pending step had been counted as accepted; -1: restart after restart)
                     kap = (T)0; jacc = 0;
                     phaseA_restart(cur);
                     __syncthreads();
@@ -531,16 +546,37 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
                 }
             }
             phaseC(prv, par);
-            T kg = (T)0;
-            if (jacc >= C::KAPN) kg = (T)kappa_tab[jacc];
-            kap = jacc < C::KAPN ? sKap[jacc] : kg;            // speculate: the step is accepted
-            ++jacc;
-            phaseA(prv, cur);                                  // hats of iteration it + 1: the new iterate sits in prv's registers
+            if ((lrun > 0 && jacc >= lrun) || (lrun < 0 && jacc == 0)) {
+                // the run of accepted steps has reached the length of the previous run, or the last two steps were restarts (the
+                // slowly converging tail of C1 / C3 restarts every step): a restart is due (C4: right two times out of three).  Wait for the decision (~300 cycles) instead of betting a repeated A + B (~1100) on "accept".
+                __syncthreads();
+                __syncthreads();
+                const int dec = *reinterpret_cast<volatile int *>(sDec);
+                if (dec == 2) return 2;
+                pend = false;
+                if (dec == 0) {
+                    T kg = (T)0;
+                    if (jacc >= C::KAPN) kg = (T)kappa_tab[jacc];
+                    kap = jacc < C::KAPN ? sKap[jacc] : kg;
+                    ++jacc;
+                    phaseA(prv, cur);
+                } else {
+                    lrun = jacc > 0 ? jacc : -1; kap = (T)0; jacc = 0;
+                    phaseA_restart(prv);
+                }
+            } else {
+                T kg = (T)0;
+                if (jacc >= C::KAPN) kg = (T)kappa_tab[jacc];
+                kap = jacc < C::KAPN ? sKap[jacc] : kg;        // predict: the step is accepted
+                ++jacc;
+                pend = true;
+                phaseA(prv, cur);                              // hats of iteration it + 1: the new iterate sits in prv's registers
+            }
             R2P(5);
 #ifdef R2_PROF
             ++pit;
 #endif
-            return false;
+            return 0;
         };
 
         // ---- results: iterate -> S[i_cur], xbar and Delta u of the last iteration (called at each exit of the loop: the
@@ -582,10 +618,14 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             int it = 0;
 #pragma unroll 1
             for (;;) {
-                if (it >= iters) { finish(sa, it > 0, 1); break; }
-                if (iteration(sa, sb, it, 0)) { finish(sa, false, 1); break; }           // iteration it-1 stopped
-                if (it + 1 >= iters) { finish(sb, true, 0); break; }
-                if (iteration(sb, sa, it + 1, 1)) { finish(sb, false, 0); break; }       // iteration it stopped
+                if (it >= iters) { finish(sa, pend, 1); break; }
+                int r = iteration(sa, sb, it, 0);
+                if (r == 1) { finish(sa, false, 1); break; }                             // iteration it-1 stopped
+                if (r == 2) { finish(sb, false, 0); break; }                             // iteration it stopped
+                if (it + 1 >= iters) { finish(sb, pend, 0); break; }
+                r = iteration(sb, sa, it + 1, 1);
+                if (r == 1) { finish(sb, false, 0); break; }
+                if (r == 2) { finish(sa, false, 1); break; }
                 it += 2;
             }
         }
