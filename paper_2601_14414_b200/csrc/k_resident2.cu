@@ -19,17 +19,20 @@
 // element-wise step of Alg. 1 works on both rows at once with packed fp32 instructions (add/mul/fma.f32x2 on sm_100a).
 // Per iteration only five 16-element vectors per stage go through shared memory (w, t, rr out; xbar, Delta u back),
 // read with 16-byte broadcast loads; the slot stride makes those loads and the 8-byte own-row stores conflict-free.
-// c (step 4) is reduced in a fixed order: stage sums in T (xor butterfly over the group), warp sums and the sum over
-// warps in double; every thread takes the same accept / restart decision (steps 5-7) from bit-identical numbers.
+// c (step 4) is reduced in a fixed order by a dedicated REDUCER warp (the CTA's last warp, which owns no stage): every lane of
+// a stage warp stores its partial sum, the reducer adds its column over the warps (a balanced tree in T), then over the lanes
+// (butterfly), promotes the total to double and takes the accept / restart decision (steps 5-7) for the whole CTA.
 //
-// The decision is SPECULATED (round 2): steps 5-7 gate the hats of the next iteration, and the
-// reduce -> decide chain was 30 % of an iteration with nothing to overlap it.  Almost every step is accepted, so the
-// kernel forms the next hats with the momentum of an accepted step right after step 4 (own registers only), lets the
-// reduction of c ride along with phases A and B of the next iteration (independent instructions of the same warps) and
-// resolves the decision before phase C, the first point that overwrites an iterate.  A restart repeats A and B with
-// kappa = 0 (hat = new iterate needs `cur` only); a stop returns the iterate phase C has not touched.  Results are the
-// ones of the unspeculated order, bit for bit.  Two CTA barriers per iteration (xbar / Delta u slots alternate by the
-// parity of the iteration, so the stopped iteration's primal step survives the speculated phase B).
+// The decision is PREDICTED (round 2): steps 5-7 gate the hats of the next iteration, and the reduce ->
+// decide chain was 30 % of an iteration with nothing to overlap it.  Almost every step is accepted, so right after step 4 the
+// stage warps form the next hats with the momentum of an accepted step (own registers only) and run phases A and B of the
+// next iteration while the reducer sums and decides; they read the decision word before phase C, the first point that
+// overwrites an iterate.  A restart repeats A and B with kappa = 0 (hat = new iterate needs `cur` only: the previous iterate
+// is dead from phase A on); a stop returns the iterate phase C has not touched.  When a restart is DUE (the run of accepted
+// steps has reached the length of the previous run, or the last two steps were restarts) the stage warps wait for the
+// decision (~300 cycles) instead of betting a repeated A + B (~1100) on "accept".  Results are those of the unpredicted
+// order, bit for bit.  Two CTA barriers per iteration (xbar / Delta u slots alternate by the parity of the iteration, so the
+// stopped iteration's primal step survives the predicted phase B).
 #include <algorithm>
 #include <cstdio>
 
