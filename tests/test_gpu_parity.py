@@ -659,3 +659,18 @@ def test_error_paths(pimpc):
     assert e.value.code == pimpc.EINVAL
     A[0, 1, 0, 0] = 1.0
     s.set_stages(A, np.ones((1, 3, 2, 1))); s.solve(2); s.sync()      # the handle recovers
+
+
+def test_measure_peaks_on_chip_rates_and_latencies(pimpc):
+    """pimpc_measure_peaks (SURVEY 8(d) "measure both with an FMA-chain microbenchmark"): the pipe rates bench.py reports
+    the RESIDENT engine against, and the latencies of a dependent instruction that DESIGN.md section 6 argues with.  Wide
+    sanity bands only (any Blackwell part): the numbers are measured, not asserted to be B200's."""
+    pk = pimpc.measure_peaks()
+    assert pk["sm_count"] >= 1
+    assert 10.0 < pk["ffma_tflops"] < 200.0 and 10.0 < pk["ffma2_tflops"] < 200.0
+    assert 0.5 < pk["dfma_tflops"] < 100.0
+    assert 5e3 < pk["smem_gbs"] < 1e5
+    assert 2.0 <= pk["lat_ffma2_cycles"] <= 12.0
+    assert pk["lat_ffma2_cycles"] < pk["lat_dadd_cycles"] <= 80.0
+    assert 10.0 <= pk["lat_shfl_cycles"] <= 60.0 and 15.0 <= pk["lat_lds_cycles"] <= 60.0
+    assert 1.0 <= pk["lds128_bcast_cycles"] <= 4.5           # between the 128 B/clk of distinct data and a full 4-wavefront load
