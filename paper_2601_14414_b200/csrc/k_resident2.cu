@@ -179,11 +179,11 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
         // ---- [A_k B_k] of every stage of the instance -> the stage's slot (the area that later holds G_k), padded, by ONE
         // coalesced cooperative load of the whole CTA: the per-solve prologue then forms U, J_k and G_k from shared memory
         // (per-lane rolled loops over global memory made the prologue 0.67 ms of C4's 7.15 ms kernel)
-        for (int i0 = tid; i0 < NS * NXP * ROWP; i0 += 4 * blockDim.x) {
+        for (int e0 = tid; e0 < NS * NXP * ROWP; e0 += 4 * blockDim.x) {
             T v[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {                      // four independent loads in flight per thread
-                const int i = i0 + u * blockDim.x;
+                const int i = e0 + u * blockDim.x;
                 const int ks = i / (NXP * ROWP), q = i - ks * (NXP * ROWP), r = q / ROWP, c = q - r * ROWP;
                 v[u] = (T)0;
                 if (ks < N && r < nx && c < NBP) {
@@ -194,7 +194,7 @@ k_res2(const Prob<T> p, const double *__restrict__ alpha_tab, const double *__re
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int i = i0 + u * blockDim.x;
+                const int i = e0 + u * blockDim.x;
                 if (i < NS * NXP * ROWP) { const int ks = i / (NXP * ROWP); sBlk[(size_t)(ks + 1) * SS + OG + (i - ks * (NXP * ROWP))] = v[u]; }
             }
         }
