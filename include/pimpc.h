@@ -42,7 +42,7 @@ enum {
     PIMPC_ENGINE_AUTO = 0,
     PIMPC_ENGINE_STAGED = 1,   /* one launch per step of Alg. 1 per iteration; any nx,nu; the A/B baseline */
     PIMPC_ENGINE_RESIDENT = 2, /* one CTA per instance, all stage data on-chip for every iteration      */
-    PIMPC_ENGINE_STREAM = 3,   /* persistent CTAs stream per-stage blobs HBM->smem (bulk async copies)   */
+    PIMPC_ENGINE_STREAM = 3,   /* persistent CTAs stream per-stage blobs HBM->smem (bulk async copies); nx <= 50, nu <= 15 */
     PIMPC_ENGINE_COOP = 4      /* cooperative grid, data resident in smem, one grid barrier per iteration */
 };
 

@@ -121,20 +121,25 @@ __global__ void __launch_bounds__(128) k_pack(const Prob<T> p, T *__restrict__ b
     T *out = blob + ((size_t)b * (N + 1) + (j + 1)) * C::BLOB;
     const bool hasH = j >= 0, hasN = j + 1 <= N - 1;
     const size_t sj = (size_t)b * N + (hasH ? j : 0), sn = (size_t)b * N + (hasN ? j + 1 : 0);
-    const T *H = p.H + sj * NB * NB, *A = p.A + sn * NX * NX, *B = p.B + sn * NX * NU, *M = p.M + sn * NU * NU;
+    // the caller's shape nx <= NX, nu <= NU sits inside the instantiated one: pad rows and columns are zero (and stay zero)
+    const int nx = p.nx, nu = p.nu, nb = p.nb;
+    auto gix = [&](int i) -> int { return i < NX ? (i < nx ? i : -1) : (i - NX < nu ? nx + (i - NX) : -1); };
+    const T *H = p.H + sj * nb * nb, *A = p.A + sn * nx * nx, *B = p.B + sn * nx * nu, *M = p.M + sn * nu * nu;
     for (int idx = threadIdx.x; idx < C::BLOB; idx += blockDim.x) {
         T v = (T)0;
         if (idx < C::OAB) {
             const int s = idx / NB, i = idx - s * NB;
             int c = i + s; if (c >= NB) c -= NB;
-            if (hasH) v = H[i * NB + c];
+            const int gi = gix(i), gc = gix(c);
+            if (hasH && gi >= 0 && gc >= 0) v = H[gi * nb + gc];
         } else if (idx < C::OM) {
             const int q = idx - C::OAB, r = q / NB, c = q - r * NB;
-            if (hasN) v = c < NX ? A[r * NX + c] : B[r * NU + (c - NX)];
+            if (hasN && r < nx) { if (c < NX) { if (c < nx) v = A[r * nx + c]; } else if (c - NX < nu) v = B[r * nu + (c - NX)]; }
         } else if (idx < C::OE) {
-            if (hasN) v = M[idx - C::OM];
+            const int q = idx - C::OM, r = q / NU, c = q - r * NU;
+            if (hasN && r < nu && c < nu) v = M[r * nu + c];
         } else if (idx < C::OE + NX) {
-            if (hasN && p.e) v = p.e[sn * NX + (idx - C::OE)];
+            if (hasN && p.e && idx - C::OE < nx) v = p.e[sn * nx + (idx - C::OE)];
         }
         out[idx] = v;
     }
@@ -156,8 +161,11 @@ struct Cursor {
 
 // EXT: per-stage boxes / linear terms or a general convex set are present (pimpc_set_stage_terms, pimpc_set_tracking with
 // per-stage references, pimpc_set_constraint); the plain variant carries none of their address arithmetic or barriers.
-template <typename T, int NX, int NU, bool EXT>
-__global__ void __launch_bounds__(SCfg<T, NX, NU>::NT)
+// PAD: the caller's shape nx <= NX, nu <= NU runs INSIDE this instantiation: blobs and the on-chip vectors are padded (pad
+// rows / columns zero, zero boxes, zero iterates: they run the same instructions and stay exactly zero), the records and the
+// caller's vectors in HBM keep the real shape and are indexed through gix().  The exact shapes compile without any of it.
+template <typename T, int NX, int NU, bool EXT, bool PAD>
+__global__ void __launch_bounds__(SCfg<T, NX, NU>::NT, PAD ? (1024 / SCfg<T, NX, NU>::NT > 2 ? 1024 / SCfg<T, NX, NU>::NT : 2) : 1)
 k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ partial, const int iters, const int nslot, const int span)
 {
     using C = SCfg<T, NX, NU>;
@@ -181,6 +189,9 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
     const bool has_du = p.has_du != 0, has_q = p.has_q != 0, gset = EXT && p.set_kind != PIMPC_SET_NONE;
     const int ci = tid % IP, prt = tid / IP;              // column index / row-range part of the column products
     const int di = tid - 4 * NX;                           // component of the dual update (threads >= 4 NX)
+    static_assert(!(EXT && PAD), "padded shapes run the plain variant only");
+    const int rnx = PAD ? p.nx : NX, rnu = PAD ? p.nu : NU, rnb = rnx + rnu, rrec = PAD ? p.rec : REC;    // the shape in HBM
+    auto gix = [&](int i) -> int { return !PAD ? i : (i < NX ? (i < rnx ? i : -1) : (i - NX < rnu ? rnx + (i - NX) : -1)); };
 
     if (tid == 0) {
         for (int s = 0; s < nslot; ++s) mbar_init(&sm.bar[s], 1);
@@ -232,13 +243,13 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
             T *dst = ring + (size_t)slot * SLOT;
             const int ks = isP ? j : j + 1;                // stage whose records are loaded
             const bool rec_ok = ks <= N - 1;
-            const uint32_t bytes = (isP ? 0u : (uint32_t)(BLOB * sizeof(T))) + (rec_ok ? 2u * REC * sizeof(T) : 0u);
+            const uint32_t bytes = (isP ? 0u : (uint32_t)(BLOB * sizeof(T))) + (rec_ok ? 2u * (uint32_t)rrec * sizeof(T) : 0u);
             mbar_expect_tx(&sm.bar[slot], bytes);
             if (!isP) bulk_g2s(dst, blob + ((size_t)L.b * N1 + (j + 1)) * BLOB, BLOB * sizeof(T), &sm.bar[slot]);
             if (rec_ok) {
                 const size_t off = p.st(L.b, ks);
-                bulk_g2s(dst + BLOB, p.S + (size_t)L.i_cur * p.buf_stride + off, REC * sizeof(T), &sm.bar[slot]);
-                bulk_g2s(dst + BLOB + REC, p.S + (size_t)L.i_prev * p.buf_stride + off, REC * sizeof(T), &sm.bar[slot]);
+                bulk_g2s(dst + BLOB, p.S + (size_t)L.i_cur * p.buf_stride + off, rrec * sizeof(T), &sm.bar[slot]);
+                bulk_g2s(dst + BLOB + REC, p.S + (size_t)L.i_prev * p.buf_stride + off, rrec * sizeof(T), &sm.bar[slot]);
             }
         };
         Cursor pc{0, 0}, cc{0, 0};
@@ -274,18 +285,18 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
 
             // ---- A: hats of stage ks from (cur, prev, kappa) (steps 6/7); w, v - beta ----
             if (tid < NB && ks <= N - 1) {
-                const int i = tid;
+                const int i = tid, gi = gix(i);
                 T h5[5];
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
-                    const T a = cu[c * NB + i], q = pv[c * NB + i];
+                    const T a = (!PAD || gi >= 0) ? cu[c * rnb + gi] : (T)0, q = (!PAD || gi >= 0) ? pv[c * rnb + gi] : (T)0;
                     h5[c] = a + kap * (a - q);
                     hs[c * NB + i] = h5[c];
                 }
                 if (has_du && i < NU) {
 #pragma unroll
                     for (int c = 0; c < 2; ++c) {
-                        const T a = cu[5 * NB + c * NU + i], q = pv[5 * NB + c * NU + i];
+                        const T a = (!PAD || i < rnu) ? cu[5 * rnb + c * rnu + i] : (T)0, q = (!PAD || i < rnu) ? pv[5 * rnb + c * rnu + i] : (T)0;
                         hs[5 * NB + c * NU + i] = a + kap * (a - q);
                     }
                 }
@@ -339,7 +350,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         if (i >= NX) g += wv[i];                                    // the [0 I] rows of Abar_{j+1}
                         h += rho * g;
                     }
-                    if (has_q) h += EXT ? p.qbar_at(b, j, i) : p.qbar[(size_t)b * p.qbar_stride + i];
+                    if (has_q) h += EXT ? p.qbar_at(b, j, i) : ((!PAD || gix(i) >= 0) ? p.qbar[(size_t)b * p.qbar_stride + gix(i)] : (T)0);
                     hv[i] = h; hv[i + NB] = h;
                 }
                 if (tid >= IP && tid < IP + NU && do_next) {
@@ -376,7 +387,10 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                 if (tid < NB) {
                     const int i = tid;
                     T x;
-                    if (first) x = i < NX ? p.x0[(size_t)b * NX + i] : p.uprev[(size_t)b * NU + (i - NX)];   // xbar_0
+                    if (first) {                                                   // xbar_0
+                        if (!PAD) x = i < NX ? p.x0[(size_t)b * NX + i] : p.uprev[(size_t)b * NU + (i - NX)];
+                        else x = i < NX ? (i < rnx ? p.x0[(size_t)b * rnx + i] : (T)0) : (i - NX < rnu ? p.uprev[(size_t)b * rnu + (i - NX)] : (T)0);
+                    }
                     else {
                         x = (T)0;
 #pragma unroll
@@ -413,7 +427,8 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                 }
                 if constexpr (!EXT) {
                     if (di >= 0 && di < NB) {
-                        const int i = di;
+                        const int i = di, gi = gix(i);
+                        const bool real = !PAD || gi >= 0;                             // pad components: zero box, nothing stored
                         if (do_next && i >= NX) {
                             bc[pn * IP + i] = xv[i] - hs[4 * NB + i];
                             avc[pn * IP + i] = duc[pn * IP + i - NX] + hs[3 * NB + i];
@@ -421,7 +436,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         if (do_dual) {
                             const T zh = hj[i], vh = hj[NB + i], thh = hj[2 * NB + i], beh = hj[3 * NB + i], lah = hj[4 * NB + i];
                             const T av = avc[pj * IP + i], bv = bc[pj * IP + i], x = xv[i];
-                            const T lo = p.lo[(size_t)b * p.bnd_stride + i], hi = p.hi[(size_t)b * p.bnd_stride + i];
+                            const T lo = real ? p.lo[(size_t)b * p.bnd_stride + gi] : (T)0, hi = real ? p.hi[(size_t)b * p.bnd_stride + gi] : (T)0;
                             const T gam = av - bv;
                             const T zn = clips(((T)2 * (x + thh + bv) + gam) * (T)(1.0 / 3.0), lo, hi);   // Thm 1 (proof form, R1)
                             const T vn = (T)0.5 * (zn + gam);
@@ -430,20 +445,21 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                             const T d5 = (zn - vn) - (zh - vh);
                             T a = d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3 + d4 * d4 + d5 * d5;
                             T *nw = p.S + (size_t)L.i_new * p.buf_stride + p.st(b, j);
-                            nw[i] = zn; nw[NB + i] = vn; nw[2 * NB + i] = thn; nw[3 * NB + i] = ben; nw[4 * NB + i] = lan;
+                            if (real) { nw[gi] = zn; nw[rnb + gi] = vn; nw[2 * rnb + gi] = thn; nw[3 * rnb + gi] = ben; nw[4 * rnb + gi] = lan; }
                             if (has_du && i >= NX) {                                   // Delta-u box copy (reading R12)
                                 const int q = i - NX;
                                 const T duq = duc[pj * IP + q], dh = hj[5 * NB + q], deh = hj[5 * NB + NU + q];
-                                const T dn = clips(duq + deh, p.dlo[(size_t)b * p.dbnd_stride + q], p.dhi[(size_t)b * p.dbnd_stride + q]);
+                                const T dn = clips(duq + deh, real ? p.dlo[(size_t)b * p.dbnd_stride + q] : (T)0,
+                                                   real ? p.dhi[(size_t)b * p.dbnd_stride + q] : (T)0);
                                 const T den = deh + duq - dn;
                                 const T e0 = den - deh, e1 = dn - dh;
                                 a += e0 * e0 + e1 * e1;
-                                nw[5 * NB + q] = dn; nw[5 * NB + NU + q] = den;
+                                if (real) { nw[5 * rnb + q] = dn; nw[5 * rnb + rnu + q] = den; }
                             }
                             acc += (double)a;
-                            if (write_x) {
-                                p.X[((size_t)b * N + j) * NB + i] = x;
-                                if (i >= NX) p.DU[((size_t)b * N + j) * NU + (i - NX)] = duc[pj * IP + i - NX];
+                            if (write_x && real) {
+                                p.X[((size_t)b * N + j) * rnb + gi] = x;
+                                if (i >= NX) p.DU[((size_t)b * N + j) * rnu + (i - NX)] = duc[pj * IP + i - NX];
                             }
                         }
                     }
@@ -574,11 +590,11 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
 
 struct StreamPlan { int grid, nslot; size_t smem; };
 
-template <typename T, int NX, int NU, bool EXT>
+template <typename T, int NX, int NU, bool EXT, bool PAD>
 int plan_stream(pimpc_s *h, StreamPlan *pl)
 {
     using C = SCfg<T, NX, NU>;
-    auto kern = k_stream<T, NX, NU, EXT>;
+    auto kern = k_stream<T, NX, NU, EXT, PAD>;
     const size_t fixed = ((sizeof(StreamSmem) + 127) / 128) * 128 + (size_t)C::V_END * sizeof(T);
     const size_t slot = (size_t)C::SLOT * sizeof(T);
     // CTAs per SM: enough bytes in flight per SM to cover the HBM latency (>= 2 slots per CTA), several
@@ -613,12 +629,12 @@ int plan_stream(pimpc_s *h, StreamPlan *pl)
     return PIMPC_OK;
 }
 
-template <typename T, int NX, int NU, bool EXT>
+template <typename T, int NX, int NU, bool EXT, bool PAD>
 int run_stream_e(pimpc_s *h, int iters, double tol)
 {
     using C = SCfg<T, NX, NU>;
     StreamPlan pl;
-    int rc = plan_stream<T, NX, NU, EXT>(h, &pl);
+    int rc = plan_stream<T, NX, NU, EXT, PAD>(h, &pl);
     if (rc) return rc;
     int launches = 0;
     const size_t nblob = (size_t)h->batch * (h->N + 1);
@@ -641,7 +657,7 @@ int run_stream_e(pimpc_s *h, int iters, double tol)
     double *partial = h->spartial;
     int nslot = pl.nslot;
     void *args[] = {(void *)&p, (void *)&blob, (void *)&partial, (void *)&iters, (void *)&nslot, (void *)&span};
-    PIMPC_CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)k_stream<T, NX, NU, EXT>, dim3(pl.grid), dim3(C::NT), args, pl.smem, h->stream));
+    PIMPC_CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)k_stream<T, NX, NU, EXT, PAD>, dim3(pl.grid), dim3(C::NT), args, pl.smem, h->stream));
     h->info.grid = pl.grid; h->info.block = C::NT; h->info.smem_bytes = pl.smem;
     return launches + 1;
 }
@@ -649,25 +665,37 @@ int run_stream_e(pimpc_s *h, int iters, double tol)
 template <typename T, int NX, int NU>
 int run_stream_t(pimpc_s *h, int iters, double tol)
 {
-    return has_stage_terms(h) ? run_stream_e<T, NX, NU, true>(h, iters, tol) : run_stream_e<T, NX, NU, false>(h, iters, tol);
+    return has_stage_terms(h) ? run_stream_e<T, NX, NU, true, false>(h, iters, tol) : run_stream_e<T, NX, NU, false, false>(h, iters, tol);
 }
 
 // (nx, nu) with a STREAM instantiation: the three BASELINE.json shapes and the paper's Table I shapes
 #define PIMPC_STREAM_SHAPES(X) X(4, 2) X(12, 4) X(48, 12) X(10, 3) X(20, 6) X(30, 10) X(50, 15)
+// containers of every other shape with nx <= 50, nu <= 15 (plain variant: no general set, no per-stage terms), smallest first:
+// the caller's shape runs inside the first one that holds it (template flag PAD)
+#define PIMPC_STREAM_CONTAINERS(X) X(12, 4) X(20, 6) X(30, 10) X(48, 12) X(50, 15)
 
-bool stream_shape(const pimpc_s *h)
+bool stream_exact(const pimpc_s *h)
 {
 #define X(NX_, NU_) if (h->nx == NX_ && h->nu == NU_) return true;
     PIMPC_STREAM_SHAPES(X)
 #undef X
     return false;
 }
+bool stream_container(const pimpc_s *h)
+{
+    if (has_stage_terms(h)) return false;
+#define X(NX_, NU_) if (h->nx <= NX_ && h->nu <= NU_) return true;
+    PIMPC_STREAM_CONTAINERS(X)
+#undef X
+    return false;
+}
+bool stream_shape(const pimpc_s *h) { return stream_exact(h) || stream_container(h); }
 
 } // namespace
 
 bool stream_supported(const pimpc_s *h, std::string *why)
 {
-    if (!stream_shape(h)) { if (why) *why = "no STREAM instantiation for this (nx, nu)"; return false; }
+    if (!stream_shape(h)) { if (why) *why = "no STREAM instantiation holds this (nx, nu) (nx <= 50, nu <= 15; general sets and per-stage terms: exact shapes only)"; return false; }
     const long long S_tot = (long long)h->batch * (h->N + 1);
     const long long grid = std::min<long long>(S_tot, h->sm_count);
     if ((S_tot / grid + 1) / (h->N + 1) + 2 > 16) { if (why) *why = "too many short instances per CTA"; return false; }
@@ -681,6 +709,11 @@ int run_stream(pimpc_s *h, int iters, double tol)
 #define X(NX_, NU_) \
     if (h->nx == NX_ && h->nu == NU_) return d ? run_stream_t<double, NX_, NU_>(h, iters, tol) : run_stream_t<float, NX_, NU_>(h, iters, tol);
     PIMPC_STREAM_SHAPES(X)
+#undef X
+#define X(NX_, NU_) \
+    if (h->nx <= NX_ && h->nu <= NU_) \
+        return d ? run_stream_e<double, NX_, NU_, false, true>(h, iters, tol) : run_stream_e<float, NX_, NU_, false, true>(h, iters, tol);
+    PIMPC_STREAM_CONTAINERS(X)
 #undef X
     h->errmsg = "STREAM engine not applicable";
     return PIMPC_EINVAL;

@@ -152,6 +152,41 @@ def test_stream_engine_paper_table1_shapes(oracle, pimpc, shape, grid, dtype):
     parity.check_properties(p, dtype, g)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("grid", [0, 3])
+@pytest.mark.parametrize("shape", [(3, 1, 19, 3), (7, 4, 13, 2), (13, 2, 11, 2), (16, 4, 9, 2), (25, 8, 7, 2), (41, 13, 5, 1)])
+def test_stream_engine_any_shape_inside_a_container(oracle, pimpc, shape, grid, dtype):
+    """Shapes without an instantiation of their own run INSIDE the smallest container that holds them ((12, 4), (20, 6),
+    (30, 10), (50, 15); template flag PAD): padded blobs and on-chip vectors, real-shape records and caller vectors.  All
+    optional terms on; AUTO must not fall back to the five-launches-per-iteration STAGED engine for them."""
+    nx, nu, N, batch = shape
+    p = wl.random_ltv(nx, nu, N, batch, seed=nx * 5 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
+                      qbar=True, bounds=0.8, du_bound=0.5)
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="stream", iters=100, tol=0.0, opts=_tune(grid=grid))
+    assert g["info"]["engine"] == pimpc.ENGINE_STREAM
+    parity.check_properties(p, dtype, g)
+    if nx > 12 or nu > 4:                                 # (beyond the register / shared-memory resident engines' shapes)
+        g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="auto", iters=100, tol=0.0)
+        assert g["info"]["engine"] == pimpc.ENGINE_STREAM
+
+
+def test_stream_engine_container_early_stop_warm_start_and_no_bounds(oracle, pimpc):
+    p = wl.random_ltv(9, 5, 12, 3, seed=91, affine=True, bounds=None, du_bound=None)
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="stream", iters=200, tol=0.0)
+    assert "D" not in g
+    p = wl.random_ltv(14, 3, 10, 2, seed=92, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
+    p.iters, p.tol = 400, 3e-2                          # stops early on some instances (the oracle's iteration counts are compared)
+    g, worst, nrep = parity.check(oracle, pimpc, p, "f64", engine="stream")
+    assert np.any(g["res"]["converged"] == 1)
+    s = pimpc.Solver(p.nx, p.nu, p.N, p.batch, dtype="f64", engine="stream")
+    s.set_problem(p); s.solve(40)
+    warm = {k: s.get_state(k) for k in ("Z", "V", "TH", "BE", "LA", "D", "DE")}
+    s.solve(25)
+    for b in range(p.batch):
+        o = parity.oracle_run(oracle, p, "f64", b, iters=25, tol=0.0, warm=warm)
+        assert parity.relerr(s.get_state("Z")[b], o.Z) <= 1e-9
+
+
 @pytest.mark.parametrize("grid", [0, 5])
 def test_stream_engine_unbounded_and_plain_admm(oracle, pimpc, grid):
     p = wl.random_ltv(4, 2, 9, 2, seed=77, affine=True, bounds=None, du_bound=None)
