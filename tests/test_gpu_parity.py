@@ -709,3 +709,35 @@ def test_measure_peaks_on_chip_rates_and_latencies(pimpc):
     assert pk["lat_ffma2_cycles"] < pk["lat_dadd_cycles"] <= 80.0
     assert 10.0 <= pk["lat_shfl_cycles"] <= 60.0 and 15.0 <= pk["lat_lds_cycles"] <= 60.0
     assert 1.0 <= pk["lds128_bcast_cycles"] <= 4.5           # between the 128 B/clk of distinct data and a full 4-wavefront load
+
+
+@pytest.mark.parametrize("iters", [1, 2, 3, 4, 7])
+@pytest.mark.parametrize("engine,dtype,shape", [("resident", "f32", (12, 4, 50, 3)), ("resident", "f32", (12, 4, 9, 2)),
+                                                ("resident", "f64", (4, 2, 20, 2)), ("coop", "f32", (12, 4, 40, 1)),
+                                                ("coop", "f64", (4, 2, 23, 1))])
+def test_predicted_decision_short_runs(oracle, pimpc, engine, dtype, shape, iters):
+    """The engines that predict the accept / restart decision unroll their loop by two and resolve a decision one phase
+    late: every exit (odd / even counts, the first iterations, a pending decision at the end) must return the oracle's
+    iterate, primal step, history and counters."""
+    nx, nu, N, batch = shape
+    p = wl.random_ltv(nx, nu, N, batch, seed=nx + N + iters, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
+    for opts in ((None,) if engine == "resident" else (None, _coop(cluster=0), _coop(lookahead=-1))):
+        g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine=engine, iters=iters, tol=0.0, opts=opts)
+        assert np.all(g["res"]["iters"] == iters)
+
+
+@pytest.mark.parametrize("engine,dtype,shape", [("resident", "f32", (12, 4, 50, 4)), ("resident", "f64", (4, 2, 20, 3)),
+                                                ("coop", "f64", (12, 4, 40, 1)), ("coop", "f32", (4, 2, 23, 1))])
+def test_predicted_decision_stop_at_every_early_iteration(oracle, pimpc, engine, dtype, shape):
+    """Early stop (step 5) right at iterations 1, 2, 3, ...: the tolerance is set just above the oracle's c of that
+    iteration, so the stop is found while the next iteration's phases already run on a predicted momentum."""
+    nx, nu, N, batch = shape
+    p = wl.random_ltv(nx, nu, N, batch, seed=17 + nx, affine=True, u_prev=True, bounds=0.8, du_bound=0.5)
+    o = parity.oracle_run(oracle, p, dtype, 0, iters=12, tol=0.0)
+    for stop_at in (1, 2, 3, 5, 8):
+        c = np.asarray(o.c_hist)
+        if not (c[stop_at - 1] < np.min(c[:stop_at - 1], initial=np.inf)):
+            continue                                      # c must fall below the tolerance for the first time there
+        p.iters, p.tol = 12, float(c[stop_at - 1]) * 1.0005
+        g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine=engine)
+        assert int(g["res"]["iters"][0]) == stop_at and int(g["res"]["converged"][0]) == 1
