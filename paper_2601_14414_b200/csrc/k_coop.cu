@@ -690,7 +690,9 @@ struct CoopPlan { int grid, spg, threads, slots; size_t smem; int cluster; };
 
 // Horizons up to this length run as ONE cluster of 16 CTAs (B200, C3 generator, us per iteration, cluster vs 64 CTAs over
 // L2: fp32 N=100 1.24 / 2.34, 200 1.42 / 2.25, 400 1.83 / 2.58, 700 2.57 / 2.55; fp64 N=100 1.56 / 2.45, 200 1.91 / 2.57,
-// 400 2.75 / 2.70); beyond it the ranges per CTA get too long and more CTAs exchanging through L2 win.
+// 400 2.75 / 2.70); beyond it the ranges per CTA get too long and more CTAs exchanging through L2 win.  The (20, 8)
+// instantiation never takes the cluster by itself: a stage costs about twice as much there and 16 CTAs are too few
+// ((20, 6) fp64, cluster vs L2: N=20 2.19 / 1.85, 50 2.31 / 1.83, 100 2.78 / 1.94; fp32 N=200 4.53 / 2.37).
 constexpr int CL_MAXN_F32 = 600, CL_MAXN_F64 = 350;
 
 template <typename T, int NX, int NU>
@@ -698,24 +700,40 @@ bool plan_coop(const pimpc_s *h, CoopPlan *pl, std::string *why)
 {
     using C = OCfg<T, NX, NU>;
     const int gmax = std::min(h->sm_count, 32 * C::MAXJ);
-    // ranges of >= 16 stages until 64 CTAs are busy, then as many CTAs as SMs (measured: the exchange grows with the grid)
-    int grid = std::min(gmax, std::max((h->N + 15) / 16, std::min(h->N, 64)));
+    // at least 64 CTAs, then ranges of >= 10 stages, then as many CTAs as SMs (measured: the exchange grows with the grid;
+    // C3 generator N=1000, 64 / 100 / 125 / 148 CTAs: fp32 1.92 / 1.89 / 2.06 / 2.12, fp64 2.37 / 2.15 / 2.28 / 2.33 us)
+    // (the (20, 8) instantiation: ranges of >= 4 stages, a stage costs more than the exchange there: (20, 6) fp64 N=500
+    // 64 / 100 / 125 / 148 CTAs 3.02 / 2.51 / 2.34 / 2.40 us per iteration)
+    constexpr int RMIN = NX <= 12 ? 10 : 4;
+    int grid = std::min(gmax, std::max((h->N + RMIN - 1) / RMIN, std::min(h->N, 64)));
     // short horizons: ONE cluster of <= 16 CTAs exchanging through distributed shared memory (opts.tune.cluster = -1
     // disables, = n forces n CTAs; automatic: 16 while N <= CL_MAXN)
     const int cl_opt = h->tune.cluster;
-    int cluster = cl_opt != 0 ? std::min(std::max(cl_opt, 0), C::CLMAX) : (h->N <= (sizeof(T) == 4 ? CL_MAXN_F32 : CL_MAXN_F64) ? C::CLMAX : 0);
-    if (cluster > 0) { cluster = std::min(cluster, h->N); grid = cluster; }
-    const int gforce = h->tune.grid;                           // fewer CTAs = longer ranges per CTA
-    if (gforce > 0) { grid = std::min(grid, gforce); if (cluster) cluster = grid; }
-    const int L = (h->N + grid - 1) / grid;                    // longest range
-    const int slots = L + 2, gpw = 32 / C::LPS;
-    const int spg_max = sizeof(T) == 8 ? 1 : 2;
-    int spg = std::min(spg_max, std::max(1, h->tune.stages_per_group));         // stages per lane group
-    while (spg <= spg_max && ((slots + spg - 1) / spg + gpw - 1) / gpw > 31) ++spg;
-    if (spg > spg_max) { if (why) *why = "horizon too long for the register-resident iterates of the COOP engine"; return false; }
-    const int ncw = ((slots + spg - 1) / spg + gpw - 1) / gpw;
-    const size_t smem = C::smem_bytes(slots, (ncw + 1) * 32);
-    if (smem > h->smem_optin) { if (why) *why = "stage matrices of a CTA's range do not fit in shared memory"; return false; }
+    const int grid_l2 = grid;
+    int cluster = cl_opt != 0 ? std::min(std::max(cl_opt, 0), C::CLMAX) : (NX <= 12 && h->N <= (sizeof(T) == 4 ? CL_MAXN_F32 : CL_MAXN_F64) ? C::CLMAX : 0);
+    int spg = 1, ncw = 0, slots = 0;
+    size_t smem = 0;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        grid = grid_l2;
+        if (cluster > 0) { cluster = std::min(cluster, h->N); grid = cluster; }
+        const int gforce = h->tune.grid;                       // fewer CTAs = longer ranges per CTA
+        if (gforce > 0) { grid = cluster ? std::min(grid, gforce) : std::min(std::min(gmax, h->N), gforce); if (cluster) cluster = grid; }
+        const int L = (h->N + grid - 1) / grid;                // longest range
+        const int gpw = 32 / C::LPS;
+        slots = L + 2;
+        const int spg_max = sizeof(T) == 8 ? 1 : 2;
+        spg = std::min(spg_max, std::max(1, h->tune.stages_per_group));         // stages per lane group
+        while (spg <= spg_max && ((slots + spg - 1) / spg + gpw - 1) / gpw > 31) ++spg;
+        const bool fits_regs = spg <= spg_max;
+        ncw = fits_regs ? ((slots + spg - 1) / spg + gpw - 1) / gpw : 0;
+        smem = fits_regs ? C::smem_bytes(slots, (ncw + 1) * 32) : 0;
+        if (fits_regs && smem <= h->smem_optin) break;
+        // an AUTOMATIC cluster of 16 whose ranges are too long for one CTA (wide shapes): more CTAs exchanging through L2
+        if (attempt == 0 && cluster > 0 && cl_opt == 0 && h->tune.grid <= 0) { cluster = 0; continue; }
+        if (why) *why = fits_regs ? "stage matrices of a CTA's range do not fit in shared memory"
+                                  : "horizon too long for the register-resident iterates of the COOP engine";
+        return false;
+    }
     pl->grid = grid; pl->spg = spg; pl->threads = (ncw + 1) * 32; pl->slots = slots; pl->smem = smem; pl->cluster = cluster;
     return true;
 }
@@ -789,20 +807,22 @@ int run_coop_t(pimpc_s *h, int iters, double tol)
     return n < 0 ? n : n + launches;
 }
 
-// padded shapes with an instantiation: (4, 4) and (12, 4); any nx <= 12, nu <= 4 runs inside the smallest that holds it
-bool coop_shape(const pimpc_s *h) { return h->nx <= 12 && h->nu <= 4; }
-bool coop_small(const pimpc_s *h) { return h->nx <= 4; }
+// padded shapes with an instantiation, smallest first: (4, 4), (12, 4), (20, 8) (one row per lane: nx + nu <= 32)
+bool coop_shape(const pimpc_s *h) { return h->nx <= 20 && h->nu <= 8; }
+int coop_class(const pimpc_s *h) { return (h->nx <= 4 && h->nu <= 4) ? 0 : ((h->nx <= 12 && h->nu <= 4) ? 1 : 2); }
 
 } // namespace
 
 bool coop_supported(const pimpc_s *h, std::string *why)
 {
     if (h->batch != 1) { if (why) *why = "COOP engine is for batch = 1"; return false; }
-    if (!coop_shape(h)) { if (why) *why = "no COOP instantiation holds this (nx, nu) (nx <= 12, nu <= 4)"; return false; }
+    if (!coop_shape(h)) { if (why) *why = "no COOP instantiation holds this (nx, nu) (nx <= 20, nu <= 8)"; return false; }
     if (h->bnd_per_instance || h->cost_per_instance) { /* batch = 1: strides are irrelevant */ }
     CoopPlan pl;
     const bool d = h->dtype == PIMPC_F64;
-    if (!coop_small(h)) return d ? plan_coop<double, 12, 4>(h, &pl, why) : plan_coop<float, 12, 4>(h, &pl, why);
+    const int cls = coop_class(h);
+    if (cls == 2) return d ? plan_coop<double, 20, 8>(h, &pl, why) : plan_coop<float, 20, 8>(h, &pl, why);
+    if (cls == 1) return d ? plan_coop<double, 12, 4>(h, &pl, why) : plan_coop<float, 12, 4>(h, &pl, why);
     return d ? plan_coop<double, 4, 4>(h, &pl, why) : plan_coop<float, 4, 4>(h, &pl, why);
 }
 
@@ -811,6 +831,8 @@ int run_coop(pimpc_s *h, int iters, double tol)
     std::string why;
     if (!coop_supported(h, &why)) { h->errmsg = "COOP engine not applicable: " + why; return PIMPC_EINVAL; }
     const bool d = h->dtype == PIMPC_F64;
-    if (!coop_small(h)) return d ? run_coop_t<double, 12, 4>(h, iters, tol) : run_coop_t<float, 12, 4>(h, iters, tol);
+    const int cls = coop_class(h);
+    if (cls == 2) return d ? run_coop_t<double, 20, 8>(h, iters, tol) : run_coop_t<float, 20, 8>(h, iters, tol);
+    if (cls == 1) return d ? run_coop_t<double, 12, 4>(h, iters, tol) : run_coop_t<float, 12, 4>(h, iters, tol);
     return d ? run_coop_t<double, 4, 4>(h, iters, tol) : run_coop_t<float, 4, 4>(h, iters, tol);
 }

@@ -241,6 +241,28 @@ def test_coop_engine_all_options(oracle, pimpc, shape, grid, dtype, cluster):
 
 
 @pytest.mark.parametrize("cluster", [None, 0])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape,grid", [((20, 6, 31), 0), ((20, 6, 90), 7), ((16, 8, 25), 3), ((13, 5, 40), 0), ((20, 8, 12), 1),
+                                        ((20, 6, 200), 0)])
+def test_coop_engine_wide_shapes_inside_20_8(oracle, pimpc, shape, grid, dtype, cluster):
+    """Shapes with 12 < nx <= 20 or 4 < nu <= 8 -- the (20, 6) of the paper's Table I among them -- run
+    inside the (20, 8) instantiation of the COOP engine (one row per lane: 28 of the 32 lanes of a stage).  All optional
+    terms on; AUTO must pick COOP for them at batch 1.  N = 200 in fp64 is longer than the ranges 16 CTAs of a cluster hold:
+    the automatic plan then takes more CTAs exchanging through L2."""
+    nx, nu, N = shape
+    if (N, grid, dtype) == (90, 7, "f64"):
+        grid = 12                         # 13 fp64 stages of (20, 8) do not fit one CTA's shared memory
+    p = wl.random_ltv(nx, nu, N, 1, seed=nx * 3 + N, affine=True, u_prev=True, full_cost=True, wdu=True,
+                      qbar=True, bounds=0.8, du_bound=0.5)
+    g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="coop", iters=120, tol=0.0, opts=_coop(grid, cluster=cluster))
+    assert g["info"]["engine"] == pimpc.ENGINE_COOP
+    parity.check_properties(p, dtype, g)
+    if grid == 0 and cluster is None:
+        g, worst, nrep = parity.check(oracle, pimpc, p, dtype, engine="auto", iters=120, tol=0.0)
+        assert g["info"]["engine"] == pimpc.ENGINE_COOP
+
+
+@pytest.mark.parametrize("cluster", [None, 0])
 @pytest.mark.parametrize("grid", [3, 0])
 def test_coop_engine_two_stages_per_group_fp32(oracle, pimpc, grid, cluster):
     p = wl.random_ltv(12, 4, 100, 1, seed=5, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
