@@ -54,15 +54,15 @@ enum { PIMPC_X = 0, PIMPC_Z = 1, PIMPC_V = 2, PIMPC_TH = 3, PIMPC_BE = 4, PIMPC_
  * change WHAT is computed, only how the stages are spread over CTAs / lanes; the parity tests use them to reach every
  * code path (ranges that split instances, ragged ranges, single-CTA runs) on small problems. */
 typedef struct {
-    int grid;             /* STREAM, COOP: at most this many CTAs (fewer CTAs = longer stage ranges per CTA)       */
+    int grid;             /* STREAM: at most this many CTAs; COOP: this many (<= N, <= SMs; fewer = longer ranges per CTA) */
     int ctas_per_sm;      /* STREAM: resident CTAs per SM                                                          */
     int ring_slots;       /* STREAM: at most this many slots in the bulk-copy ring                                 */
     int stages_per_group; /* COOP: stages per lane group (1 or 2)                                                  */
     int cluster;          /* COOP: -1 = never one thread-block cluster (exchange through L2), n > 0 = cluster of
                              n CTAs (<= 16), 0 = automatic (one cluster for short horizons)                       */
     int rows_per_lane;    /* RESIDENT: matrix rows per lane (1 or 2; 2 only where instantiated)                    */
-    int lookahead;        /* COOP: 1 = prepare the next iteration for both candidate momenta while the partial sums
-                             of c travel, -1 = never, 0 = automatic                                 */
+    int lookahead;        /* COOP: >= 0 = run the next iteration's phases on the PREDICTED accept / restart decision
+                             while the partial sums of c travel (same bits), -1 = wait for the decision */
     int reserved_;
 } pimpc_tune;
 
