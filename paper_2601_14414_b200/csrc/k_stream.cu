@@ -165,7 +165,7 @@ struct Cursor {
 // rows / columns zero, zero boxes, zero iterates: they run the same instructions and stay exactly zero), the records and the
 // caller's vectors in HBM keep the real shape and are indexed through gix().  The exact shapes compile without any of it.
 template <typename T, int NX, int NU, bool EXT, bool PAD>
-__global__ void __launch_bounds__(SCfg<T, NX, NU>::NT, PAD ? (1024 / SCfg<T, NX, NU>::NT > 2 ? 1024 / SCfg<T, NX, NU>::NT : 2) : 1)
+__global__ void __launch_bounds__(SCfg<T, NX, NU>::NT, PAD ? (1024 / SCfg<T, NX, NU>::NT > 2 ? 1024 / SCfg<T, NX, NU>::NT : 2) : 0)
 k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ partial, const int iters, const int nslot, const int span)
 {
     using C = SCfg<T, NX, NU>;
