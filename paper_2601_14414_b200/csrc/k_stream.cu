@@ -32,7 +32,12 @@ template <typename T, int NX, int NU>
 struct SCfg {
     static constexpr int NB = NX + NU;
     static constexpr int NS = NB / 2 + 1;                 // circulant rows s = 0..NB/2:  C[s][i] = H[i][(i+s) % NB]
-    static constexpr int OC = 0, OAB = NS * NB, OM = OAB + NX * NB, OE = OM + NU * NU;
+    // NB % 4 == 0: the symmetric H_j is stored as its lower triangle of 4 x 4 blocks instead (block t = I(I+1)/2 + J, J <= I;
+    // row a of block t at [a][t][0..3], so consecutive lanes read consecutive 16-byte words): one thread multiplies a block
+    // and its transpose from registers -- 6 16-byte loads per 32 FMAs where the circulant order needs 64 4-byte loads
+    static constexpr bool BLKH = NB % 4 == 0;
+    static constexpr int NBK = NB / 4, NBLK = NBK * (NBK + 1) / 2;
+    static constexpr int OC = 0, OAB = BLKH ? 16 * NBLK : NS * NB, OM = OAB + NX * NB, OE = OM + NU * NU;
     static constexpr int BLOB = round4(OE + NX);          // elements per blob'
     static constexpr int REC = round4(5 * NB + 2 * NU);   // iterate record (same as Prob<T>::rec)
     static constexpr int SLOT = BLOB + 2 * REC;           // ring slot: blob', cur record, prev record
@@ -41,16 +46,21 @@ struct SCfg {
     static constexpr int NPART = NT / IP;                 // column-products are split into NPART row ranges
     static constexpr int NW = NT / 32;
     static constexpr int MAXI = 16;                       // instances a CTA's range may touch
+    // register budget: 64 per thread in fp32 (1024 resident threads: 4 CTAs of 256), 128 in fp64 (512 threads: shared memory
+    // holds 2 CTAs of the wide shapes anyway).  Without a bound ptxas picks what it likes (124 registers once in fp32: -27 %)
+    static constexpr int MINB = (sizeof(T) == 4 ? 1024 : 512) / NT > 2 ? (sizeof(T) == 4 ? 1024 : 512) / NT : 2;
     static_assert(NT >= 4 * NX + NB && NPART >= 1 && IP + NU <= NT, "thread mapping");
+    static_assert(!BLKH || (NBLK <= NT - 32 && NU <= 32), "one thread per 4 x 4 block of H, the last warp for M rhs");
     // fixed shared-memory vectors (elements of T)
     static constexpr int V_HAT = 0;                       // [2][REC] hats of stages j, j+1 (ping-pong on stage parity)
     static constexpr int V_W = V_HAT + 2 * REC;           // [IP] w_{j+1}
     static constexpr int V_D = V_W + IP;                  // [IP] vhat - betahat of stage j+1
-    static constexpr int V_GP = V_D + IP;                 // [NPART][IP] partial Abar^T w
+    static constexpr int V_H = V_D + IP;                  // [2 NB] h_j twice (circulant wrap)
+    static constexpr int V_GP = V_H + 2 * NB;             // [NPART][IP] partial Abar^T w
     static constexpr int V_RP = V_GP + NPART * IP;        // [NPART][IP] partial Bbar^T d (u columns)
-    static constexpr int V_H = V_RP + NPART * IP;         // [2 NB] h_j twice (circulant wrap)
-    static constexpr int V_XP = V_H + 2 * NB;             // [NPART][IP] partial H h
-    static constexpr int V_X = V_XP + NPART * IP;         // [IP] xbar_{j+1}
+    static constexpr int V_XP = V_RP + NPART * IP;        // [NPART][IP] partial H h; BLKH: [NBK][NB] from V_GP on (gp, rp are dead by then)
+    static constexpr int XP_LEN = BLKH && NBK * NB > 3 * NPART * IP ? NBK * NB - 2 * NPART * IP : NPART * IP;
+    static constexpr int V_X = V_XP + XP_LEN;         // [IP] xbar_{j+1}
     static constexpr int V_RHS = V_X + IP;                // [IP] rhs of the Delta-u update
     static constexpr int V_DU = V_RHS + IP;               // [2][IP] Delta u carry
     static constexpr int V_B = V_DU + 2 * IP;             // [2][IP] b carry
@@ -111,6 +121,12 @@ __device__ __forceinline__ void ld4s(const double *p, double (&o)[4])
     o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
 }
 
+__device__ __forceinline__ void st4s(float *p, const float (&v)[4]) { *reinterpret_cast<float4 *>(p) = make_float4(v[0], v[1], v[2], v[3]); }
+__device__ __forceinline__ void st4s(double *p, const double (&v)[4])
+{
+    *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]); *reinterpret_cast<double2 *>(p + 2) = make_double2(v[2], v[3]);
+}
+
 // ---- pack: blob'_j of every (instance, j = -1..N-1), once per solve after the cache kernel ----------
 template <typename T, int NX, int NU>
 __global__ void __launch_bounds__(128) k_pack(const Prob<T> p, T *__restrict__ blob)
@@ -128,8 +144,16 @@ __global__ void __launch_bounds__(128) k_pack(const Prob<T> p, T *__restrict__ b
     for (int idx = threadIdx.x; idx < C::BLOB; idx += blockDim.x) {
         T v = (T)0;
         if (idx < C::OAB) {
-            const int s = idx / NB, i = idx - s * NB;
-            int c = i + s; if (c >= NB) c -= NB;
+            int i, c;
+            if constexpr (C::BLKH) {
+                const int a = idx / (4 * C::NBLK), t = (idx >> 2) % C::NBLK, bq = idx & 3;
+                int I = 0; while ((I + 1) * (I + 2) / 2 <= t) ++I;
+                i = 4 * I + a; c = 4 * (t - I * (I + 1) / 2) + bq;
+            } else {
+                const int s = idx / NB;
+                i = idx - s * NB;
+                c = i + s; if (c >= NB) c -= NB;
+            }
             const int gi = gix(i), gc = gix(c);
             if (hasH && gi >= 0 && gc >= 0) v = H[gi * nb + gc];
         } else if (idx < C::OM) {
@@ -165,7 +189,7 @@ struct Cursor {
 // rows / columns zero, zero boxes, zero iterates: they run the same instructions and stay exactly zero), the records and the
 // caller's vectors in HBM keep the real shape and are indexed through gix().  The exact shapes compile without any of it.
 template <typename T, int NX, int NU, bool EXT, bool PAD>
-__global__ void __launch_bounds__(SCfg<T, NX, NU>::NT, PAD ? (1024 / SCfg<T, NX, NU>::NT > 2 ? 1024 / SCfg<T, NX, NU>::NT : 2) : 0)
+__global__ void __launch_bounds__(SCfg<T, NX, NU>::NT, SCfg<T, NX, NU>::MINB)
 k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ partial, const int iters, const int nslot, const int span)
 {
     using C = SCfg<T, NX, NU>;
@@ -176,7 +200,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
     T *vec = reinterpret_cast<T *>(smem_raw + ((sizeof(StreamSmem) + 127) / 128) * 128);
     T *ring = vec + C::V_END;
     T *hat = vec + C::V_HAT, *wv = vec + C::V_W, *dv = vec + C::V_D, *gp = vec + C::V_GP, *rp = vec + C::V_RP;
-    T *hv = vec + C::V_H, *xp = vec + C::V_XP, *xv = vec + C::V_X, *rhs = vec + C::V_RHS, *duc = vec + C::V_DU;
+    T *hv = vec + C::V_H, *xp = vec + (C::BLKH ? C::V_GP : C::V_XP), *xv = vec + C::V_X, *rhs = vec + C::V_RHS, *duc = vec + C::V_DU;
     T *bc = vec + C::V_B, *avc = vec + C::V_AV;
 
     cg::grid_group grid = cg::this_grid();
@@ -190,6 +214,9 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
     const int ci = tid % IP, prt = tid / IP;              // column index / row-range part of the column products
     const int di = tid - 4 * NX;                           // component of the dual update (threads >= 4 NX)
     static_assert(!(EXT && PAD), "padded shapes run the plain variant only");
+    int bI = 0;                                            // BLKH: this thread's 4 x 4 block (bI, bJ) of the lower triangle of H
+    if (C::BLKH && tid < C::NBLK) while ((bI + 1) * (bI + 2) / 2 <= tid) ++bI;
+    const int bJ = tid - bI * (bI + 1) / 2;
     const int rnx = PAD ? p.nx : NX, rnu = PAD ? p.nu : NU, rnb = rnx + rnu, rrec = PAD ? p.rec : REC;    // the shape in HBM
     auto gix = [&](int i) -> int { return !PAD ? i : (i < NX ? (i < rnx ? i : -1) : (i - NX < rnu ? rnx + (i - NX) : -1)); };
 
@@ -362,7 +389,34 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                     rhs[q] = r;
                 }
                 __syncthreads();
-                // ---- D: xbar_{j+1} = H_j h_j, H stored once: C[s][i] = H[i][(i+s) % NB] ----
+                // ---- D: xbar_{j+1} = H_j h_j.  BLKH: H stored as the lower triangle of 4 x 4 blocks; the thread of block (I, J)
+                // adds B h_J to segment I and B^T h_I to segment J, as partial xp[other block index][component] (each written once;
+                // phase E sums them in ascending order: a fixed order that does not depend on the thread mapping); the last warp
+                // forms Delta u_{j+1} = M rhs meanwhile.  Else: circulant order C[s][i] = H[i][(i+s) % NB] ----
+                if constexpr (C::BLKH) {
+                    if (tid < C::NBLK && !first) {
+                        T m[4][4], hI[4], hJ[4], y[4];
+#pragma unroll
+                        for (int a = 0; a < 4; ++a) ld4s(Cb + (a * C::NBLK + tid) * 4, m[a]);
+                        ld4s(hv + 4 * bJ, hJ);
+                        ld4s(hv + 4 * bI, hI);
+#pragma unroll
+                        for (int a = 0; a < 4; ++a) y[a] = ((m[a][0] * hJ[0] + m[a][1] * hJ[1]) + m[a][2] * hJ[2]) + m[a][3] * hJ[3];
+                        st4s(xp + bJ * NB + 4 * bI, y);
+                        if (bI != bJ) {
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) y[c] = ((m[0][c] * hI[0] + m[1][c] * hI[1]) + m[2][c] * hI[2]) + m[3][c] * hI[3];
+                            st4s(xp + bI * NB + 4 * bJ, y);
+                        }
+                    }
+                    if (tid >= C::NT - 32 && tid - (C::NT - 32) < NU && do_next) {
+                        const int q = tid - (C::NT - 32);
+                        T d = (T)0;
+#pragma unroll
+                        for (int k2 = 0; k2 < NU; ++k2) d += Mb[q * NU + k2] * rhs[k2];
+                        duc[pn * IP + q] = d;
+                    }
+                } else
                 if (ci < NB && !first) {
                     T a0 = (T)0, a1 = (T)0;
                     constexpr int QD = (C::NS + NPART - 1) / NPART;
@@ -391,6 +445,12 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         if (!PAD) x = i < NX ? p.x0[(size_t)b * NX + i] : p.uprev[(size_t)b * NU + (i - NX)];
                         else x = i < NX ? (i < rnx ? p.x0[(size_t)b * rnx + i] : (T)0) : (i - NX < rnu ? p.uprev[(size_t)b * rnu + (i - NX)] : (T)0);
                     }
+                    else if constexpr (C::BLKH) {
+                        T x0_ = xp[i], x1_ = C::NBK > 1 ? xp[NB + i] : (T)0;
+#pragma unroll
+                        for (int o = 2; o < C::NBK; ++o) { if (o & 1) x1_ += xp[o * NB + i]; else x0_ += xp[o * NB + i]; }
+                        x = C::NBK > 1 ? x0_ + x1_ : x0_;
+                    }
                     else {
                         x = (T)0;
 #pragma unroll
@@ -398,7 +458,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                     }
                     xv[i] = x;
                 }
-                if (tid >= IP && tid < IP + NU && do_next) {
+                if (!C::BLKH && tid >= IP && tid < IP + NU && do_next) {
                     const int q = tid - IP;
                     T d = (T)0;
 #pragma unroll
