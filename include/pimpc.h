@@ -255,6 +255,34 @@ int pimpc_sync(pimpc_t h);
 int pimpc_get_info(pimpc_t h, pimpc_info *info);
 const char *pimpc_last_error(pimpc_t h);
 
+/* ---- allocation-free entry point ----------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (stream capture, tight serving loops, harnesses that forbid it).
+ * r_prim2[b] = rho ||F p + G q - h||^2 of an iterate the caller holds: the primal-residual half of c^{i+1}
+ * (the consensus constraints of Problem (11)), the same definition, accumulation
+ * type (double) and chunking as pimpc_result.r_prim2 of pimpc_get, without a handle.  No cudaMalloc / cudaFree / allocating
+ * library call, no host synchronisation: two kernel launches on `stream` (a cudaStream_t of the CURRENT device, NULL =
+ * default stream).
+ *
+ * Every pointer is a DEVICE pointer to a dense array of element type `dtype` (PIMPC_F64 | PIMPC_F32); r_prim2 is
+ * double[batch] in device memory whatever the dtype.  Inputs are only read; the caller owns everything.
+ *   A [batch][N][nx][nx], B [batch][N][nx][nu], e [batch][N][nx] or NULL (= 0)           stage data
+ *   x0 [batch][nx], u_prev [batch][nu] or NULL (= 0)                                     xbar_0
+ *   X, Z, V [batch][N][nx+nu], DU [batch][N][nu], D [batch][N][nu] or NULL (no Delta-u box)
+ *                                                  the layouts pimpc_get_state(PIMPC_X / _Z / _V / _DU / _D) returns
+ * The per-CTA partial sums live in a file-scope __device__ array of PIMPC_NOALLOC_MAX_PARTS doubles (256 KiB, held by
+ * every GPU that loads the library until the process exits).  Limit: batch <= PIMPC_NOALLOC_MAX_PARTS (an instance
+ * gets min(64, N (nx+nu) / 2048, PIMPC_NOALLOC_MAX_PARTS / batch) >= 1 partials); beyond it, or with a bad dtype /
+ * shape / NULL required pointer: PIMPC_EINVAL, nothing launched.  PIMPC_ECUDA: the scratch address could not be
+ * resolved or a launch failed.  pimpc_noalloc_last_error() returns the message of the calling thread's last failure.
+ * ALL calls on a device share the array: calls that may overlap on the GPU (different streams, other host threads)
+ * race and give wrong sums -- order them on one stream or with events.  The array keeps the previous call's contents;
+ * nothing in it has to start at zero (every partial a call reads was written by that call's first kernel). */
+#define PIMPC_NOALLOC_MAX_PARTS 32768
+int pimpc_rprim2_noalloc(int dtype, int nx, int nu, int N, int batch, const void *A, const void *B, const void *e,
+                         const void *x0, const void *u_prev, const void *X, const void *DU, const void *Z, const void *V,
+                         const void *D, double rho, double *r_prim2, void *stream);
+const char *pimpc_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -93,6 +93,8 @@ SYMBOLS = {
     "pimpc_sync": (_i, [_vp]),
     "pimpc_get_info": (_i, [_vp, ctypes.POINTER(pimpc_info)]),
     "pimpc_last_error": (ctypes.c_char_p, [_vp]),
+    "pimpc_rprim2_noalloc": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _d, _vp, _vp]),
+    "pimpc_noalloc_last_error": (ctypes.c_char_p, []),
 }
 
 _lib = None
@@ -321,6 +323,21 @@ def measure_peaks(stream=None) -> dict:
     if rc != OK:
         raise PimpcError(rc, "pimpc_measure_peaks failed")
     return {f: getattr(pk, f) for f, _ in pimpc_peaks._fields_ if f != "pad_"}
+
+
+NOALLOC_MAX_PARTS = 32768      # PIMPC_NOALLOC_MAX_PARTS of include/pimpc.h
+
+
+def rprim2_noalloc(dtype, nx, nu, N, batch, A, B, e, x0, u_prev, X, DU, Z, V, D, rho, r_prim2, stream=None):
+    """pimpc_rprim2_noalloc: r_prim2[b] of the iterate in the caller's DEVICE arrays (torch tensors or raw device pointers),
+    into the caller's device double[batch]; no allocation, no synchronisation, asynchronous on `stream`.  Calls on one
+    device share a static scratch array: do not let them overlap on the GPU."""
+    rc = load().pimpc_rprim2_noalloc(F64 if dtype == "f64" else (F32 if dtype == "f32" else int(dtype)), nx, nu, N, batch,
+                                     _ptr(A), _ptr(B), _ptr(e), _ptr(x0), _ptr(u_prev), _ptr(X), _ptr(DU), _ptr(Z), _ptr(V),
+                                     _ptr(D), float(rho), _ptr(r_prim2), stream)
+    if rc != OK:
+        raise PimpcError(rc, load().pimpc_noalloc_last_error().decode())
+    return r_prim2
 
 
 def version() -> str:
