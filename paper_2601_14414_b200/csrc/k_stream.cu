@@ -286,11 +286,32 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
 
         double acc = 0.0;                                  // this thread's part of sum ||.||^2 of the current segment
         int slot = 0;
+        // per-segment state, reloaded when a segment starts (uniform branch): the segment record, the instance, its momentum
+        // and -- plain variant -- this thread's bounds and linear term, which are the same for every stage of the instance
+        Seg sg = sm.seg[0];
+        int li = 0, b = 0;
+        T kap = (T)0, lo_c = (T)0, hi_c = (T)0, dlo_c = (T)0, dhi_c = (T)0, qb_c = (T)0;
         for (int n = 0; n < total; ++n) {
-            const Seg sg = sm.seg[cc.sg];
-            const int li = sg.b;
+            if (cc.o == 0) {
+                sg = sm.seg[cc.sg];
+                li = sg.b;
+                b = sm.inst[li].b;
+                kap = (T)sm.inst[li].kappa;
+                if constexpr (!EXT) {
+                    if (di >= 0 && di < NB) {
+                        const int gi = gix(di);
+                        const bool real = !PAD || gi >= 0;
+                        lo_c = real ? p.lo[(size_t)b * p.bnd_stride + gi] : (T)0;
+                        hi_c = real ? p.hi[(size_t)b * p.bnd_stride + gi] : (T)0;
+                        if (has_du && di >= NX) {
+                            dlo_c = real ? p.dlo[(size_t)b * p.dbnd_stride + (di - NX)] : (T)0;
+                            dhi_c = real ? p.dhi[(size_t)b * p.dbnd_stride + (di - NX)] : (T)0;
+                        }
+                    }
+                    if (has_q && tid < NB) qb_c = (!PAD || gix(tid) >= 0) ? p.qbar[(size_t)b * p.qbar_stride + gix(tid)] : (T)0;
+                }
+            }
             const LInst &L = sm.inst[li];
-            const int b = L.b;
             const bool isP = sg.pstep && cc.o == 0;
             const int so = cc.o - sg.pstep;                // index of the S step inside the segment
             const int j = isP ? sg.j0 : sg.j0 + so;
@@ -298,7 +319,6 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
             const bool do_dual = !isP && j >= 0 && !(sg.halo && so == 0);
             const bool last_of_seg = cc.o == sg.nsteps - 1;
             const bool do_next = has_next && !last_of_seg;
-            const T kap = (T)L.kappa;
             const T *sl = ring + (size_t)slot * SLOT;
             const T *Cb = sl + C::OC, *AB = sl + C::OAB, *Mb = sl + C::OM, *Eb = sl + C::OE;
             const T *cu = sl + BLOB, *pv = cu + REC;
@@ -377,7 +397,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         if (i >= NX) g += wv[i];                                    // the [0 I] rows of Abar_{j+1}
                         h += rho * g;
                     }
-                    if (has_q) h += EXT ? p.qbar_at(b, j, i) : ((!PAD || gix(i) >= 0) ? p.qbar[(size_t)b * p.qbar_stride + gix(i)] : (T)0);
+                    if (has_q) h += EXT ? p.qbar_at(b, j, i) : qb_c;
                     hv[i] = h; hv[i + NB] = h;
                 }
                 if (tid >= IP && tid < IP + NU && do_next) {
@@ -496,7 +516,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                         if (do_dual) {
                             const T zh = hj[i], vh = hj[NB + i], thh = hj[2 * NB + i], beh = hj[3 * NB + i], lah = hj[4 * NB + i];
                             const T av = avc[pj * IP + i], bv = bc[pj * IP + i], x = xv[i];
-                            const T lo = real ? p.lo[(size_t)b * p.bnd_stride + gi] : (T)0, hi = real ? p.hi[(size_t)b * p.bnd_stride + gi] : (T)0;
+                            const T lo = lo_c, hi = hi_c;
                             const T gam = av - bv;
                             const T zn = clips(((T)2 * (x + thh + bv) + gam) * (T)(1.0 / 3.0), lo, hi);   // Thm 1 (proof form, R1)
                             const T vn = (T)0.5 * (zn + gam);
@@ -509,8 +529,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                             if (has_du && i >= NX) {                                   // Delta-u box copy (reading R12)
                                 const int q = i - NX;
                                 const T duq = duc[pj * IP + q], dh = hj[5 * NB + q], deh = hj[5 * NB + NU + q];
-                                const T dn = clips(duq + deh, real ? p.dlo[(size_t)b * p.dbnd_stride + q] : (T)0,
-                                                   real ? p.dhi[(size_t)b * p.dbnd_stride + q] : (T)0);
+                                const T dn = clips(duq + deh, dlo_c, dhi_c);
                                 const T den = deh + duq - dn;
                                 const T e0 = den - deh, e1 = dn - dh;
                                 a += e0 * e0 + e1 * e1;
@@ -594,7 +613,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                 }
                 acc = 0.0;
             }
-            cc.next(sm.seg);
+            if (++cc.o >= sg.nsteps) { cc.o = 0; ++cc.sg; }
         }
         // new records were written through the generic proxy and are read next iteration by bulk copies
         __threadfence();
