@@ -46,6 +46,10 @@ struct SCfg {
     static constexpr int NPART = NT / IP;                 // column-products are split into NPART row ranges
     static constexpr int NW = NT / 32;
     static constexpr int MAXI = 16;                       // instances a CTA's range may touch
+    // the thread that issues the bulk copies: lane 0 of a warp with no work in phases A, C and E (the refill of a slot then
+    // overlaps phase A of the next step instead of preceding it on warp 0)
+    static constexpr int PROD = NT >= 128 ? 96 : (NT >= 64 ? 32 : 0);
+    static_assert(PROD == 0 || PROD >= NB, "the producer's warp has no hats to form");
     // register budget: 64 per thread in fp32 (1024 resident threads: 4 CTAs of 256), 128 in fp64 (512 threads: shared memory
     // holds 2 CTAs of the wide shapes anyway).  Without a bound ptxas picks what it likes (124 registers once in fp32: -27 %)
     static constexpr int MINB = (sizeof(T) == 4 ? 1024 : 512) / NT > 2 ? (sizeof(T) == 4 ? 1024 : 512) / NT : 2;
@@ -261,7 +265,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
         __syncthreads();
         const int total = sm.total;
 
-        // producer: thread 0 issues the bulk copies of step n into slot n % nslot
+        // producer: thread PROD issues the bulk copies of step n into slot n % nslot
         auto issue = [&](const Cursor &cu, int slot) {
             const Seg sg = sm.seg[cu.sg];
             const LInst &L = sm.inst[sg.b];
@@ -281,7 +285,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
         };
         Cursor pc{0, 0}, cc{0, 0};
         int issued = 0;
-        if (tid == 0)
+        if (tid == C::PROD)
             for (; issued < nslot && issued < total; ++issued) { issue(pc, issued); pc.next(sm.seg); }
 
         double acc = 0.0;                                  // this thread's part of sum ||.||^2 of the current segment
@@ -597,7 +601,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                 }
             }
             __syncthreads();                                 // slot and ping-pong vectors are free again
-            if (tid == 0 && issued < total) { issue(pc, slot); pc.next(sm.seg); ++issued; }
+            if (tid == C::PROD && issued < total) { issue(pc, slot); pc.next(sm.seg); ++issued; }
             if (++slot == nslot) slot = 0;
             // ---- end of a segment: this CTA's part of c of the instance (fixed order) ----
             if (last_of_seg) {
