@@ -33,7 +33,7 @@ struct SCfg {
     static constexpr int NB = NX + NU;
     static constexpr int NS = NB / 2 + 1;                 // circulant rows s = 0..NB/2:  C[s][i] = H[i][(i+s) % NB]
     // NB % 4 == 0: the symmetric H_j is stored as its lower triangle of 4 x 4 blocks instead (block t = I(I+1)/2 + J, J <= I;
-    // row a of block t at [a][t][0..3], so consecutive lanes read consecutive 16-byte words): one thread multiplies a block
+    // row a of block t at [a][t][0..3] (fp64: [a][half][t][0..1]), so consecutive lanes read consecutive 16-byte words): one thread multiplies a block
     // and its transpose from registers -- 6 16-byte loads per 32 FMAs where the circulant order needs 64 4-byte loads
     static constexpr bool BLKH = NB % 4 == 0;
     static constexpr int NBK = NB / 4, NBLK = NBK * (NBK + 1) / 2;
@@ -125,6 +125,14 @@ __device__ __forceinline__ void ld4s(const double *p, double (&o)[4])
     o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
 }
 
+// row a of 4 x 4 block t of H (see SCfg::BLKH): consecutive lanes read consecutive 16-byte words in either precision
+__device__ __forceinline__ void ldblk(const float *Cb, int a, int nblk, int t, float (&o)[4]) { ld4s(Cb + (a * nblk + t) * 4, o); }
+__device__ __forceinline__ void ldblk(const double *Cb, int a, int nblk, int t, double (&o)[4])
+{
+    const double2 lo = *reinterpret_cast<const double2 *>(Cb + ((2 * a) * nblk + t) * 2);
+    const double2 hi = *reinterpret_cast<const double2 *>(Cb + ((2 * a + 1) * nblk + t) * 2);
+    o[0] = lo.x; o[1] = lo.y; o[2] = hi.x; o[3] = hi.y;
+}
 __device__ __forceinline__ void st4s(float *p, const float (&v)[4]) { *reinterpret_cast<float4 *>(p) = make_float4(v[0], v[1], v[2], v[3]); }
 __device__ __forceinline__ void st4s(double *p, const double (&v)[4])
 {
@@ -150,7 +158,10 @@ __global__ void __launch_bounds__(128) k_pack(const Prob<T> p, T *__restrict__ b
         if (idx < C::OAB) {
             int i, c;
             if constexpr (C::BLKH) {
-                const int a = idx / (4 * C::NBLK), t = (idx >> 2) % C::NBLK, bq = idx & 3;
+                // 16-byte words of consecutive blocks are adjacent: [a][t][0..3] in fp32, [a][half][t][0..1] in fp64
+                constexpr int EW = 16 / (int)sizeof(T), HW = 4 / EW;          // elements per word, words per block row
+                const int wq = idx / EW, t = wq % C::NBLK, ah = wq / C::NBLK;
+                const int a = ah / HW, bq = (ah % HW) * EW + idx % EW;
                 int I = 0; while ((I + 1) * (I + 2) / 2 <= t) ++I;
                 i = 4 * I + a; c = 4 * (t - I * (I + 1) / 2) + bq;
             } else {
@@ -421,7 +432,7 @@ k_stream(const Prob<T> p, const T *__restrict__ blob, double *__restrict__ parti
                     if (tid < C::NBLK && !first) {
                         T m[4][4], hI[4], hJ[4], y[4];
 #pragma unroll
-                        for (int a = 0; a < 4; ++a) ld4s(Cb + (a * C::NBLK + tid) * 4, m[a]);
+                        for (int a = 0; a < 4; ++a) ldblk(Cb, a, C::NBLK, tid, m[a]);
                         ld4s(hv + 4 * bJ, hJ);
                         ld4s(hv + 4 * bI, hI);
 #pragma unroll
