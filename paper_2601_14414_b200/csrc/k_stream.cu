@@ -3,7 +3,8 @@
 // persistent CTAs each own a contiguous range of (instance, stage) pairs and, every iteration,
 // stream one packed blob per stage HBM -> shared memory with bulk asynchronous copies (TMA 1-D,
 // cp.async.bulk + mbarrier ring), so HBM sees exactly the algorithmic bytes:
-//   blob'_j = { H_j (symmetric, stored once in circulant order), [A_{j+1} B_{j+1}], M_{j+1}, e_{j+1} }
+//   blob'_j = { H_j (symmetric, stored once: lower triangle of 4 x 4 blocks if nb % 4 == 0, else circulant order),
+//               [A_{j+1} B_{j+1}], M_{j+1}, e_{j+1} }
 //   + the (current, previous) iterate records of stage j+1 in, the new record of stage j out.
 // The regrouping (H of stage j with A, B, M of stage j+1) makes every step need ONE blob:
 //   step j:  g = Abar_{j+1}^T w_{j+1},  rhs/du/av of stage j+1          (Alg. 1 step 1)
