@@ -187,6 +187,31 @@ def test_stream_engine_container_early_stop_warm_start_and_no_bounds(oracle, pim
         assert parity.relerr(s.get_state("Z")[b], o.Z) <= 1e-9
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(48, 12, 160, 6), (30, 10, 90, 3), (20, 6, 70, 4)])
+def test_stream_engine_repeated_runs_are_bit_identical(pimpc, shape, dtype):
+    """Two runs of the same solve on the same launch shape (several stage steps per CTA, ranges that split instances, every
+    ring slot reused many times): every iterate, the primal step and the history of c bit for bit.  The stage step reuses
+    its shared-memory vectors across phases (the H h partials overlay the column-product partials) and slots across
+    steps: a missing barrier or a copy landing early would show here as a difference between runs."""
+    nx, nu, N, batch = shape
+    p = wl.random_ltv(nx, nu, N, batch, seed=N, affine=True, u_prev=True, qbar=True, bounds=0.8, du_bound=0.5)
+    s = pimpc.Solver(nx, nu, N, batch, dtype=dtype, engine="stream", rho=p.rho, history=60)
+    s.set_problem(p)
+    runs = []
+    for _ in range(3):
+        s.reset()
+        s.solve(60, 0.0)
+        runs.append(({k: s.get_state(k).copy() for k in ("X", "DU", "Z", "V", "TH", "BE", "LA", "D", "DE")}, s.get_history()[0].copy()))
+    assert s.get_info()["engine"] == pimpc.ENGINE_STREAM
+    s.close()
+    for st, hist in runs[1:]:
+        for k, v in st.items():
+            np.testing.assert_array_equal(v, runs[0][0][k], err_msg=k)
+        np.testing.assert_array_equal(hist, runs[0][1])
+    assert np.isfinite(runs[0][1]).all() and (runs[0][1][:, -1] < runs[0][1][:, 0]).all()
+
+
 @pytest.mark.parametrize("grid", [0, 5])
 def test_stream_engine_unbounded_and_plain_admm(oracle, pimpc, grid):
     p = wl.random_ltv(4, 2, 9, 2, seed=77, affine=True, bounds=None, du_bound=None)
