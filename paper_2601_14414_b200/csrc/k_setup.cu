@@ -103,6 +103,130 @@ __global__ void __launch_bounds__(256) k_setup(Prob<T> p, const int *__restrict_
     else if (!ok && tid == 0) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
 }
 
+// ---- a0 for 16 < nb <= 64: FOUR threads per matrix row, LP / 4 columns of the row in the registers of each, one CTA of
+// 4 LP threads per (instance, stage); the matrix is padded to LP x LP with identity rows.  The pivot row and the pivot column
+// of each exchange step travel through a double-buffered shared-memory line (one CTA barrier per pivot).  k_setup above keeps
+// the matrix in shared memory (three loads, an integer division and a store per FMA, two barriers per pivot): C5, 128 000
+// stages of 60 x 60, took 70.9 ms there.  Same exchange steps as gj_rows (rank-1 update, column p overwritten).
+template <typename T, int LP>
+__global__ void __launch_bounds__(LP * 4) k_setup_rows(Prob<T> p, const int *__restrict__ list)
+{
+    // LPK: a row line with every quarter (the CPT columns of one thread) shifted by 16 bytes more than the one before: the four
+    // 16-byte words a warp-wide load touches (one per quarter) then sit in different banks (unshifted they are 128 bytes apart:
+    // ncu counted 73 % of the shared-memory wavefronts as bank conflicts)
+    constexpr int CPT = LP / 4, TS = LP + 1, NT = LP * 4, LPK = LP + 8;
+    static_assert(CPT % 2 == 0, "16-byte alignment of the exchange lines");
+    extern __shared__ __align__(16) double sm[];
+    double *Ssm = sm;                                          // [LP][TS] after the inversion; before: [nx][LPK] rows of [A_{k+1} B_{k+1}]
+    double *rowb = sm + LP * LPK, *colb = rowb + 2 * LPK;      // [2][LPK], [2][LP] (parity of the pivot)
+    const int nx = p.nx, nu = p.nu, nb = p.nb, N = p.N;
+    const int sflat = list ? list[blockIdx.x] : (int)blockIdx.x;
+    const int b = sflat / N, k = sflat - b * N;
+    const int tid = threadIdx.x, i = tid >> 2, q = tid & 3, j0 = q * CPT, j0k = q * (CPT + 2);
+    const int ik = i + 2 * (i / CPT);                          // position of column i in a shifted line
+    const bool last = (k == N - 1);
+    const T *A1 = p.A + ((size_t)b * N + (last ? k : k + 1)) * nx * nx;
+    const T *B1 = p.B + ((size_t)b * N + (last ? k : k + 1)) * nx * nu;
+    const T *Qx = (last && p.P) ? p.P + (size_t)b * p.cost_stride_q : p.Q + (size_t)b * p.cost_stride_q;
+    const T *Rx = p.R + (size_t)b * p.cost_stride_r;
+    const double rho = p.rho;
+    bool finite = true;
+
+    // H_k = (Qbar + rho I + rho Abar_{k+1}^T Abar_{k+1})^-1, k < N-1;  (Qbar_N + rho I)^-1, k = N-1
+    for (int idx = tid; idx < nx * LP; idx += NT) {            // rows of [A_{k+1} B_{k+1}] as doubles, zero-padded to LP columns
+        const int r = idx / LP, c = idx - r * LP;
+        const double v = c < nx ? (double)A1[r * nx + c] : (c < nb ? (double)B1[r * nu + (c - nx)] : 0.0);
+        if (!isfinite(v)) finite = false;
+        Ssm[r * LPK + c + 2 * (c / CPT)] = v;
+    }
+    __syncthreads();
+    double S[CPT];
+    const double rl = last ? 0.0 : rho;                        // the terminal stage has no Abar_{k+1} term
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+        const int j = j0 + c;
+        double v = 0.0;
+        if (i < nb && j < nb) {
+            if (i < nx && j < nx) v = (double)Qx[i * nx + j];
+            else if (i >= nx && j >= nx) v = (double)Rx[(i - nx) * nu + (j - nx)];
+            if (i == j) v += rho + (i >= nx ? rl : 0.0);        // rho I and the [0 I] rows of rho Abar^T Abar
+        } else if (i == j) v = 1.0;                             // pad rows: identity
+        S[c] = v;
+    }
+    for (int r = 0; r < nx; ++r) {                              // + rho [A B]^T [A B]
+        const double ai = rl * Ssm[r * LPK + ik];
+#pragma unroll
+        for (int c = 0; c < CPT; c += 2) {
+            const double2 v = *reinterpret_cast<const double2 *>(Ssm + r * LPK + j0k + c);
+            S[c] = fma(ai, v.x, S[c]); S[c + 1] = fma(ai, v.y, S[c + 1]);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < CPT; ++c)
+        if (!isfinite(S[c])) finite = false;
+
+    // exchange steps; the pivot loop is unrolled over a quarter so that column pv has a compile-time index in its owners' registers
+    bool ok = true;
+    for (int qq = 0; qq < 4; ++qq) {
+#pragma unroll
+        for (int c0 = 0; c0 < CPT; ++c0) {
+            const int pv = qq * CPT + c0;
+            if (pv < nb) {                                      // uniform over the CTA
+                double *rb = rowb + (pv & 1) * LPK, *cb = colb + (pv & 1) * LP;
+                if (i == pv) {
+#pragma unroll
+                    for (int c = 0; c < CPT; c += 2) *reinterpret_cast<double2 *>(rb + j0k + c) = make_double2(S[c], S[c + 1]);
+                }
+                if (q == qq) cb[i] = S[c0];
+                __syncthreads();                                // the lines of the previous pivot have the other parity
+                const double piv = rb[qq * (CPT + 2) + c0];
+                if (!(piv > 0.0) || !isfinite(piv)) ok = false;
+                const double inv = 1.0 / piv;
+                const double f = (i == pv) ? 1.0 - inv : cb[i] * inv;
+#pragma unroll
+                for (int c = 0; c < CPT; c += 2) {
+                    const double2 r2 = *reinterpret_cast<const double2 *>(rb + j0k + c);
+                    S[c] = fma(-f, r2.x, S[c]); S[c + 1] = fma(-f, r2.y, S[c + 1]);
+                }
+                if (q == qq) S[c0] = (i == pv) ? inv : -f;
+            }
+        }
+    }
+    __syncthreads();                                            // everybody is done with the rows of [A B] (first pivot at the latest) and the lines
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) Ssm[i * TS + j0 + c] = S[c];
+    __syncthreads();
+    T *Hk = p.H + ((size_t)b * N + k) * nb * nb;
+    for (int idx = tid; idx < nb * nb; idx += NT) {
+        const int i2 = idx / nb, j2 = idx - i2 * nb;
+        Hk[idx] = (T)(0.5 * (Ssm[i2 * TS + j2] + Ssm[j2 * TS + i2]));   // exactly symmetric
+    }
+    __syncthreads();
+
+    // M_k = (B_k^T B_k + I [+ Wdu/rho] [+ I])^-1  so that J_k = M_k Bbar_k^T  (R12, R13)
+    const T *Bk = p.B + ((size_t)b * N + k) * nx * nu;
+    const T *Ak = p.A + ((size_t)b * N + k) * nx * nx;
+    for (int idx = tid; idx < nx * nx; idx += NT)
+        if (!isfinite((double)Ak[idx])) finite = false;
+    for (int idx = tid; idx < nu * nu; idx += NT) {
+        const int i2 = idx / nu, j2 = idx - i2 * nu;
+        double v = (i2 == j2) ? 1.0 : 0.0;
+        for (int r = 0; r < nx; ++r) v += (double)Bk[r * nu + i2] * (double)Bk[r * nu + j2];
+        if (p.Wdu) v += (double)p.Wdu[(size_t)b * p.cost_stride_r + idx] / rho;
+        if (p.has_du && i2 == j2) v += 1.0;
+        if (!isfinite(v)) finite = false;
+        Ssm[idx] = v;
+    }
+    ok = gj_invert(Ssm, colb, rowb, nu) && ok;
+    T *Mk = p.M + ((size_t)b * N + k) * nu * nu;
+    for (int idx = tid; idx < nu * nu; idx += NT) {
+        const int i2 = idx / nu, j2 = idx - i2 * nu;
+        Mk[idx] = (T)(0.5 * (Ssm[idx] + Ssm[j2 * nu + i2]));
+    }
+    if (!finite) atomicOr(p.err, PIMPC_DEVERR_NONFINITE);
+    else if (!ok) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
+}
+
 // ---- a0 for small stages (nb <= 32): one lane per matrix row, a group of LPS lanes per (instance, stage) --------
 // Row i of the SPD matrix lives in the registers of lane i (double precision whatever the dtype); the pivot
 // row of each Gauss-Jordan exchange step is broadcast through a per-group shared-memory row.  Same arithmetic
@@ -502,6 +626,13 @@ static int setup_t(pimpc_s *h, const int *list, int nlist)
     if (h->nx == 12 && h->nu == 4) return setup_small_t<T, 12, 4>(h, list, nlist);
     if (h->nx == 4 && h->nu == 2) return setup_small_t<T, 4, 2>(h, list, nlist);
     Prob<T> p = make_prob<T>(h, 0.0);
+    if (h->nb > 16 && h->nb <= 64 && h->nu <= 32) {            // rows in registers, four threads per row
+        const long long nst = list ? nlist : (long long)h->batch * h->N;
+        if (h->nb <= 32) k_setup_rows<T, 32><<<(unsigned)nst, 128, (32 * 40 + 2 * 40 + 2 * 32) * sizeof(double), h->stream>>>(p, list);
+        else k_setup_rows<T, 64><<<(unsigned)nst, 256, (64 * 72 + 2 * 72 + 2 * 64) * sizeof(double), h->stream>>>(p, list);
+        PIMPC_CUDA_TRY(h, cudaGetLastError());
+        return 1;
+    }
     const size_t smem = ((size_t)h->nb * h->nb + 2 * h->nb) * sizeof(double);
     if (smem > 48 * 1024)
         PIMPC_CUDA_TRY(h, cudaFuncSetAttribute(k_setup<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
