@@ -122,7 +122,8 @@ __global__ void __launch_bounds__(LP * 4) k_setup_rows(Prob<T> p, const int *__r
     const int nx = p.nx, nu = p.nu, nb = p.nb, N = p.N;
     const int sflat = list ? list[blockIdx.x] : (int)blockIdx.x;
     const int b = sflat / N, k = sflat - b * N;
-    const int tid = threadIdx.x, i = tid >> 2, q = tid & 3, j0 = q * CPT, j0k = q * (CPT + 2);
+    // a warp holds 8 rows; 8 consecutive lanes share a quarter, so each quarter-warp of a 16-byte load of a row line reads ONE word
+    const int tid = threadIdx.x, i = (tid >> 5) * 8 + (tid & 7), q = (tid >> 3) & 3, j0 = q * CPT, j0k = q * (CPT + 2);
     const int ik = i + 2 * (i / CPT);                          // position of column i in a shifted line
     const bool last = (k == N - 1);
     const T *A1 = p.A + ((size_t)b * N + (last ? k : k + 1)) * nx * nx;
@@ -133,6 +134,7 @@ __global__ void __launch_bounds__(LP * 4) k_setup_rows(Prob<T> p, const int *__r
     bool finite = true;
 
     // H_k = (Qbar + rho I + rho Abar_{k+1}^T Abar_{k+1})^-1, k < N-1;  (Qbar_N + rho I)^-1, k = N-1
+#pragma unroll 4
     for (int idx = tid; idx < nx * LP; idx += NT) {            // rows of [A_{k+1} B_{k+1}] as doubles, zero-padded to LP columns
         const int r = idx / LP, c = idx - r * LP;
         const double v = c < nx ? (double)A1[r * nx + c] : (c < nb ? (double)B1[r * nu + (c - nx)] : 0.0);
