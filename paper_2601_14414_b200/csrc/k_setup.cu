@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(256) k_setup(Prob<T> p, const int *__restrict_
     else if (!ok && tid == 0) atomicOr(p.err, PIMPC_DEVERR_NOTPD);
 }
 
-// ---- a0 for 16 < nb <= 64: FOUR threads per matrix row, LP / 4 columns of the row in the registers of each, one CTA of
+// ---- a0 for 8 < nb <= 64: FOUR threads per matrix row, LP / 4 columns of the row in the registers of each, one CTA of
 // 4 LP threads per (instance, stage); the matrix is padded to LP x LP with identity rows.  The pivot row and the pivot column
 // of each exchange step travel through a double-buffered shared-memory line (one CTA barrier per pivot).  k_setup above keeps
 // the matrix in shared memory (three loads, an integer division and a store per FMA, two barriers per pivot): C5, 128 000
@@ -628,7 +628,7 @@ static int setup_t(pimpc_s *h, const int *list, int nlist)
     if (h->nx == 12 && h->nu == 4) return setup_small_t<T, 12, 4>(h, list, nlist);
     if (h->nx == 4 && h->nu == 2) return setup_small_t<T, 4, 2>(h, list, nlist);
     Prob<T> p = make_prob<T>(h, 0.0);
-    if (h->nb > 16 && h->nb <= 64 && h->nu <= 32) {            // rows in registers, four threads per row
+    if (h->nb > 8 && h->nb <= 64 && h->nu <= 32) {             // rows in registers, four threads per row (tiny matrices: k_setup below)
         const long long nst = list ? nlist : (long long)h->batch * h->N;
         if (h->nb <= 32) k_setup_rows<T, 32><<<(unsigned)nst, 128, (32 * 40 + 2 * 40 + 2 * 32) * sizeof(double), h->stream>>>(p, list);
         else k_setup_rows<T, 64><<<(unsigned)nst, 256, (64 * 72 + 2 * 72 + 2 * 64) * sizeof(double), h->stream>>>(p, list);
