@@ -242,15 +242,11 @@ __device__ __forceinline__ bool gj_rows(double (&S)[W], double *rowb, const int 
 #pragma unroll
     for (int p = 0; p < NPIV; ++p) {
         __syncwarp();
-        if (li == p) {
-            if constexpr (W % 2 == 0) {                        // 16-byte stores / broadcast loads of the pivot row
-#pragma unroll
-                for (int j = 0; j < W; j += 2) *reinterpret_cast<double2 *>(rowb + j) = make_double2(S[j], S[j + 1]);
-            } else {
-#pragma unroll
-                for (int j = 0; j < W; ++j) rowb[j] = S[j];
-            }
-        }
+        // The pivot row, from the pivot COLUMN every lane already holds at a compile-time index: the matrix is symmetric at
+        // the start (Q, R, W_du symmetric: include/pimpc.h) and an exchange step keeps S[p][j] = S[j][p] for the rows j not yet
+        // pivoted and S[p][j] = -S[j][p] for the pivoted ones (j < p).  One 8-byte store per lane instead of the owner lane's
+        // W / 2 16-byte stores (ncu: the stores were a third of the shared-memory wavefronts of this kernel).
+        rowb[li] = (li < p) ? -S[p] : S[p];
         __syncwarp();
         const double piv = rowb[p], colv = S[p];
         if (!(piv > 0.0) || !isfinite(piv)) ok = false;
