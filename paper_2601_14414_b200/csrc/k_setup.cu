@@ -175,11 +175,8 @@ __global__ void __launch_bounds__(LP * 4) k_setup_rows(Prob<T> p, const int *__r
             const int pv = qq * CPT + c0;
             if (pv < nb) {                                      // uniform over the CTA
                 double *rb = rowb + (pv & 1) * LPK, *cb = colb + (pv & 1) * LP;
-                if (i == pv) {
-#pragma unroll
-                    for (int c = 0; c < CPT; c += 2) *reinterpret_cast<double2 *>(rb + j0k + c) = make_double2(S[c], S[c + 1]);
-                }
-                if (q == qq) cb[i] = S[c0];
+                // column pv from its owners; the pivot ROW is the same numbers up to the sign of the pivoted rows (see gj_rows)
+                if (q == qq) { cb[i] = S[c0]; rb[ik] = (i < pv) ? -S[c0] : S[c0]; }
                 __syncthreads();                                // the lines of the previous pivot have the other parity
                 const double piv = rb[qq * (CPT + 2) + c0];
                 if (!(piv > 0.0) || !isfinite(piv)) ok = false;
