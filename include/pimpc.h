@@ -164,7 +164,9 @@ int pimpc_set_stage(pimpc_t h, int b, int k, const void *A_k, const void *B_k, c
 /* Bulk setter: A [batch][N][nx][nx], B [batch][N][nx][nu], e [batch][N][nx] or NULL (= keep). */
 int pimpc_set_stages(pimpc_t h, const void *A, const void *B, const void *e);
 
-/* Cost.  Q [nx][nx] = C'W_y C and R [nu][nu] = W_u symmetric PSD.
+/* Cost.  Q [nx][nx] = C'W_y C and R [nu][nu] = W_u symmetric PSD; so are P and Wdu.  The cache kernels
+ * rely on the symmetry (they read the pivot row of each exchange step from the pivot column): a non-symmetric matrix is not
+ * detected and gives a wrong cache.
  * P [nx][nx] or NULL: terminal weight used instead of Q at stage N-1 (R14; NULL = Q).
  * Wdu [nu][nu] or NULL: weight on Delta u (R13; NULL = 0).
  * qbar [nx+nu] or NULL: linear term col(C'W_y r_y, W_u r_u) (NULL = 0); replaces per-stage linear terms.
